@@ -1,0 +1,250 @@
+/*
+ * nf_oracle.c -- CPU ORACLE for the Abacus near-field force.  TEST INFRASTRUCTURE ONLY.
+ *
+ * This file is the plain, slow, double-precision statement of what the CUDA path
+ * (paper_2110_11392_b200/csrc) must compute.  It is imported only by tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs.  It shares no
+ * code, header, table or helper with the CUDA path and the product never calls it.
+ *
+ * What it follows (reference = /root/reference/PAPER.md, arXiv 2110.11392):
+ *   - near-field domain: "every cell interacting with itself and its 124 nearest neighbor
+ *     cells (for near-field radius R=2) using open boundary conditions and Newtonian
+ *     gravity, or a softened form thereof"            PAPER.md:218 (sec. 3.4.1), :62 (sec. 2.1)
+ *   - softening law, Eq. 3: F = [10 - 15u + 6u^2] r/eps_s^3 (u = r/eps_s < 1), r/r^3 else
+ *                                                     PAPER.md:132 (sec. 3.2)
+ *   - eps_s = 2.16 eps_p                              PAPER.md:143 (sec. 3.2, Fig. 4 caption :141)
+ *   - grid of K^3 (=CPD^3) cells, particles kept in grid order, offsets from cell centres
+ *                                                     PAPER.md:72 (sec. 2.2), :264 (sec. 3.5.1)
+ *   - "handles the periodic wrap" by shifting whole cells (pencil-centred coordinates)
+ *                                                     PAPER.md:232 (sec. 3.4.2)
+ * Readings where the paper is silent are those of SURVEY.md 8(c) S1-S14, listed in DESIGN.md.
+ *
+ * The near field is exact by definition (a direct sum), so the oracle IS that definition:
+ * piecewise Eq. 3 with a branch (not the GPU's min form), no blocking, no reordering beyond
+ * the loop nest "sink cell -> (a,b,c) lexicographic -> sink -> source".
+ *
+ * Parity pins (tests/test_oracle_pins.py): two-particle closed form inside/outside eps_s,
+ * cell-based cutoff, periodic wrap, one-particle-per-cell lattice => 0, momentum sum = 0,
+ * all-pairs brute force masked to near-field cell pairs, integer pair-count identity,
+ * CPD = 2R+1 => plain all-pairs, whole-cell translation, input-order invariance.
+ * Every function below is pinned; nothing here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define NFO_SPLINE_PER_PLUMMER 2.16 /* eps_s = 2.16 eps_p */
+
+int nfo_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* Scalar force law of Eq. 3: returns f such that F = f * r_vec. */
+double nfo_force_factor(double r, double eps_s) {
+    if (r < eps_s) {
+        double u = r / eps_s;
+        return (10.0 - 15.0 * u + 6.0 * u * u) / (eps_s * eps_s * eps_s);
+    }
+    return 1.0 / (r * r * r);
+}
+
+/* Plummer law, Eq. 2: f such that F = f * r_vec.  Used only by the pin that
+ * checks the 2.16 conversion against "match the small-scale Plummer force". */
+double nfo_plummer_factor(double r, double eps_p) {
+    double s = r * r + eps_p * eps_p;
+    return 1.0 / (s * sqrt(s));
+}
+
+/*
+ * Binning (PAPER.md:72 grid order; :264 offsets relative to cell centres; reading S5):
+ * per axis t = (double)x * (CPD/box); I = floor(t); cell index = I mod CPD (non-negative);
+ * offset from the cell centre, in box units, = (t - I - 0.5) * (box/CPD), kept in double.
+ * key = (cx*CPD + cy)*CPD + cz  (z fastest).
+ * Returns 0, or -1 if a position is not finite.
+ */
+int nfo_bin(const float *pos, int64_t N, int cpd, double box, int32_t *cell, double *off) {
+    const double scale = (double)cpd / box;
+    const double cellsz = box / (double)cpd;
+    int bad = 0;
+    for (int64_t i = 0; i < N; ++i) {
+        int c[3];
+        for (int k = 0; k < 3; ++k) {
+            double x = (double)pos[3 * i + k];
+            if (!isfinite(x)) { bad = 1; x = 0.0; }
+            double t = x * scale;
+            double I = floor(t);
+            double m = fmod(I, (double)cpd);
+            if (m < 0) m += (double)cpd;
+            c[k] = (int)m;
+            if (off) off[3 * i + k] = (t - I - 0.5) * cellsz;
+        }
+        cell[i] = (c[0] * cpd + c[1]) * cpd + c[2];
+    }
+    return bad ? -1 : 0;
+}
+
+/* Grid-ordered lists (CellInfo offset+count :399): stable counting sort of
+ * particle indices by cell key; within a cell, ascending original index (reading S12).
+ * offsets has ncell+1 entries; order[s] = original index of the s-th particle in grid order. */
+void nfo_cell_lists(const int32_t *cell, int64_t N, int64_t ncell, int64_t *offsets, int64_t *order) {
+    memset(offsets, 0, (size_t)(ncell + 1) * sizeof(int64_t));
+    for (int64_t i = 0; i < N; ++i) offsets[cell[i] + 1]++;
+    for (int64_t c = 0; c < ncell; ++c) offsets[c + 1] += offsets[c];
+    int64_t *cur = (int64_t *)malloc((size_t)ncell * sizeof(int64_t));
+    memcpy(cur, offsets, (size_t)ncell * sizeof(int64_t));
+    for (int64_t i = 0; i < N; ++i) order[cur[cell[i]]++] = i;
+    free(cur);
+}
+
+static inline int wrap_idx(int v, int cpd, int *image) {
+    /* v in [-cpd, 2cpd): image = floor(v/cpd) in {-1,0,1} */
+    int w = 0;
+    if (v < 0) { v += cpd; w = -1; }
+    else if (v >= cpd) { v -= cpd; w = 1; }
+    *image = w;
+    return v;
+}
+
+/* Neighbour list of one cell (reading S3): the (2R+1)^3 cells
+ * ((i+a) mod CPD, (j+b) mod CPD, (k+c) mod CPD), (a,b,c) in [-R,R]^3 lexicographic (a slowest),
+ * each with its periodic image count floor((i+a)/CPD) etc. in {-1,0,1}.  */
+void nfo_neighbors(int cpd, int R, int cellid, int32_t *ids, int8_t *image) {
+    int k = cellid % cpd, j = (cellid / cpd) % cpd, i = cellid / (cpd * cpd);
+    int n = 0;
+    for (int a = -R; a <= R; ++a)
+        for (int b = -R; b <= R; ++b)
+            for (int c = -R; c <= R; ++c) {
+                int wa, wb, wc;
+                int ia = wrap_idx(i + a, cpd, &wa), jb = wrap_idx(j + b, cpd, &wb), kc = wrap_idx(k + c, cpd, &wc);
+                ids[n] = (ia * cpd + jb) * cpd + kc;
+                image[3 * n + 0] = (int8_t)wa;
+                image[3 * n + 1] = (int8_t)wb;
+                image[3 * n + 2] = (int8_t)wc;
+                ++n;
+            }
+}
+
+/* Number of (sink, source) pairs the definition visits, q != p:
+ * sum over cells c of n_c * sum over the (2R+1)^3 neighbours c' of n_c', minus N.
+ * Counted by walking the same neighbour lists as nfo_accel (not by a closed form). */
+int64_t nfo_pair_count(const int64_t *offsets, int cpd, int R) {
+    int64_t ncell = (int64_t)cpd * cpd * cpd, total = 0, N = offsets[ncell];
+    int nn = (2 * R + 1) * (2 * R + 1) * (2 * R + 1);
+#pragma omp parallel
+    {
+        int32_t *ids = (int32_t *)malloc((size_t)nn * sizeof(int32_t));
+        int8_t *img = (int8_t *)malloc((size_t)nn * 3);
+#pragma omp for reduction(+ : total) schedule(static)
+        for (int64_t c = 0; c < ncell; ++c) {
+            int64_t nc = offsets[c + 1] - offsets[c];
+            if (nc == 0) continue;
+            nfo_neighbors(cpd, R, (int)c, ids, img);
+            int64_t s = 0;
+            for (int n = 0; n < nn; ++n) s += offsets[ids[n] + 1] - offsets[ids[n]];
+            total += nc * s;
+        }
+        free(ids);
+        free(img);
+    }
+    return total - N;
+}
+
+/*
+ * Near-field acceleration (the definition):
+ *   for each sink cell C=(i,j,k), for (a,b,c) in [-R,R]^3 lexicographic:
+ *     S = ((i+a) mod CPD, (j+b) mod CPD, (k+c) mod CPD)
+ *     for sink p in C, for source q in S, q != p:
+ *        d  = (off_q - off_p) + (a,b,c)*cell          -- x_source - x_sink, cell-pair image (S3, S6)
+ *        r2 = d.d ; if r2 == 0 continue               -- F(0) = 0 (S4)
+ *        f  = Eq. 3 with eps_s = 2.16 eps_p           -- PAPER.md:132, :143
+ *        a_p += gm * f * d                            -- attractive, gm = G*m (S7)
+ * sink_cells: list of n_sink_cells cell ids to evaluate, or NULL for all cells.
+ * acc[N][3] (double, input order) is written only for particles in evaluated cells; the
+ * caller zero-fills.  Returns the number of pairs evaluated (q != p, r2 == 0 included), or
+ * -1 on a non-finite position / bad arguments.
+ */
+int64_t nfo_accel(const float *pos, int64_t N, int cpd, int R, double eps_p, double box, double gm,
+                  const int32_t *sink_cells, int64_t n_sink_cells, double *acc, int nthreads) {
+    if (N < 0 || R < 1 || cpd < 2 * R + 1 || !(eps_p > 0) || !(box > 0)) return -1;
+    const int64_t ncell = (int64_t)cpd * cpd * cpd;
+    const double cellsz = box / (double)cpd;
+    const double eps_s = NFO_SPLINE_PER_PLUMMER * eps_p;
+    const int nn = (2 * R + 1) * (2 * R + 1) * (2 * R + 1);
+
+    int32_t *cell = (int32_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int32_t));
+    double *off = (double *)malloc((size_t)(N > 0 ? N : 1) * 3 * sizeof(double));
+    int64_t *offsets = (int64_t *)malloc((size_t)(ncell + 1) * sizeof(int64_t));
+    int64_t *order = (int64_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int64_t));
+    if (!cell || !off || !offsets || !order) { free(cell); free(off); free(offsets); free(order); return -1; }
+    if (nfo_bin(pos, N, cpd, box, cell, off) != 0) { free(cell); free(off); free(offsets); free(order); return -1; }
+    nfo_cell_lists(cell, N, ncell, offsets, order);
+
+    /* grid-ordered copy of the offsets so the inner loop streams */
+    double *so = (double *)malloc((size_t)(N > 0 ? N : 1) * 3 * sizeof(double));
+    for (int64_t s = 0; s < N; ++s) {
+        int64_t i = order[s];
+        so[3 * s + 0] = off[3 * i + 0]; so[3 * s + 1] = off[3 * i + 1]; so[3 * s + 2] = off[3 * i + 2];
+    }
+
+    const int64_t nwork = sink_cells ? n_sink_cells : ncell;
+    int64_t pairs = 0;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel
+    {
+        int32_t *ids = (int32_t *)malloc((size_t)nn * sizeof(int32_t));
+        int8_t *img = (int8_t *)malloc((size_t)nn * 3);
+#pragma omp for schedule(dynamic, 1) reduction(+ : pairs)
+        for (int64_t w = 0; w < nwork; ++w) {
+            const int C = sink_cells ? sink_cells[w] : (int)w;
+            const int64_t p0 = offsets[C], p1 = offsets[C + 1];
+            if (p0 == p1) continue;
+            nfo_neighbors(cpd, R, C, ids, img);
+            for (int64_t p = p0; p < p1; ++p) {
+                double ax = 0.0, ay = 0.0, az = 0.0;
+                const double px = so[3 * p], py = so[3 * p + 1], pz = so[3 * p + 2];
+                int n = 0;
+                for (int a = -R; a <= R; ++a)
+                    for (int b = -R; b <= R; ++b)
+                        for (int c = -R; c <= R; ++c, ++n) {
+                            const int S = ids[n];
+                            const double sx = a * cellsz, sy = b * cellsz, sz = c * cellsz;
+                            const int64_t q0 = offsets[S], q1 = offsets[S + 1];
+                            for (int64_t q = q0; q < q1; ++q) {
+                                if (q == p) continue;
+                                const double dx = (so[3 * q] - px) + sx;
+                                const double dy = (so[3 * q + 1] - py) + sy;
+                                const double dz = (so[3 * q + 2] - pz) + sz;
+                                const double r2 = dx * dx + dy * dy + dz * dz;
+                                ++pairs;
+                                if (r2 == 0.0) continue;
+                                const double r = sqrt(r2);
+                                double f;
+                                if (r < eps_s) {
+                                    const double u = r / eps_s;
+                                    f = (10.0 - 15.0 * u + 6.0 * u * u) / (eps_s * eps_s * eps_s);
+                                } else {
+                                    f = 1.0 / (r2 * r);
+                                }
+                                ax += gm * f * dx; ay += gm * f * dy; az += gm * f * dz;
+                            }
+                        }
+                const int64_t i = order[p];
+                acc[3 * i] = ax; acc[3 * i + 1] = ay; acc[3 * i + 2] = az;
+            }
+        }
+        free(ids);
+        free(img);
+    }
+    free(so); free(cell); free(off); free(offsets); free(order);
+    return pairs;
+}

@@ -1,0 +1,154 @@
+"""ctypes loader for ``nf_oracle.c`` (TEST INFRASTRUCTURE -- see the C file's header).
+
+The shared object is built with gcc on first use (``-O3 -march=native -fopenmp``, no
+``-ffast-math``) and named after a hash of the source and of the host CPU's flags, so a copy
+built on another machine is never loaded by mistake.
+"""
+from __future__ import annotations
+
+import ctypes
+import hashlib
+import os
+import subprocess
+import sys
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nf_oracle.c")
+_lib = None
+
+
+def _cpu_tag() -> str:
+    flags = ""
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("flags"):
+                    flags = line
+                    break
+    except OSError:
+        pass
+    with open(_SRC, "rb") as f:
+        src = f.read()
+    return hashlib.sha1(src + flags.encode()).hexdigest()[:12]
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, f"libnf_oracle.{_cpu_tag()}.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile ``nf_oracle.c`` with gcc (building the checker is not using it)."""
+    out = lib_path()
+    if force or not os.path.exists(out):
+        tmp = out + f".tmp{os.getpid()}"
+        cmd = ["gcc", "-O3", "-march=native", "-fopenmp", "-std=c99", "-shared", "-fPIC",
+               "-o", tmp, _SRC, "-lm"]
+        subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
+        os.replace(tmp, out)
+    return out
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        i64, i32, dbl, vp = ctypes.c_int64, ctypes.c_int, ctypes.c_double, ctypes.c_void_p
+        L.nfo_max_threads.restype = i32
+        L.nfo_force_factor.restype = dbl
+        L.nfo_force_factor.argtypes = [dbl, dbl]
+        L.nfo_plummer_factor.restype = dbl
+        L.nfo_plummer_factor.argtypes = [dbl, dbl]
+        L.nfo_bin.restype = i32
+        L.nfo_bin.argtypes = [vp, i64, i32, dbl, vp, vp]
+        L.nfo_cell_lists.restype = None
+        L.nfo_cell_lists.argtypes = [vp, i64, i64, vp, vp]
+        L.nfo_neighbors.restype = None
+        L.nfo_neighbors.argtypes = [i32, i32, i32, vp, vp]
+        L.nfo_pair_count.restype = i64
+        L.nfo_pair_count.argtypes = [vp, i32, i32]
+        L.nfo_accel.restype = i64
+        L.nfo_accel.argtypes = [vp, i64, i32, i32, dbl, dbl, dbl, vp, i64, vp, i32]
+        _lib = L
+    return _lib
+
+
+def _f32pos(pos) -> np.ndarray:
+    p = np.ascontiguousarray(pos, dtype=np.float32)
+    if p.ndim != 2 or p.shape[1] != 3:
+        raise ValueError("pos must be [N,3]")
+    return p
+
+
+def max_threads() -> int:
+    return int(_load().nfo_max_threads())
+
+
+def force_factor(r: float, eps_s: float) -> float:
+    """f with F = f * r_vec, Eq. 3."""
+    return float(_load().nfo_force_factor(float(r), float(eps_s)))
+
+
+def plummer_factor(r: float, eps_p: float) -> float:
+    """f with F = f * r_vec, Eq. 2."""
+    return float(_load().nfo_plummer_factor(float(r), float(eps_p)))
+
+
+def bin_particles(pos, cpd: int, box: float = 1.0):
+    """-> (cell[N] int32, off[N,3] float64 offsets from cell centres, box units)."""
+    p = _f32pos(pos)
+    N = p.shape[0]
+    cell = np.empty(N, dtype=np.int32)
+    off = np.empty((N, 3), dtype=np.float64)
+    rc = _load().nfo_bin(p.ctypes.data, N, cpd, float(box), cell.ctypes.data, off.ctypes.data)
+    if rc != 0:
+        raise ValueError("non-finite position")
+    return cell, off
+
+
+def cell_lists(cell: np.ndarray, cpd: int):
+    """-> (offsets[cpd^3+1] int64, order[N] int64): grid order, stable within a cell."""
+    cell = np.ascontiguousarray(cell, dtype=np.int32)
+    ncell = cpd ** 3
+    offsets = np.empty(ncell + 1, dtype=np.int64)
+    order = np.empty(cell.shape[0], dtype=np.int64)
+    _load().nfo_cell_lists(cell.ctypes.data, cell.shape[0], ncell, offsets.ctypes.data, order.ctypes.data)
+    return offsets, order
+
+
+def neighbors(cpd: int, R: int, cellid: int):
+    """-> (ids[(2R+1)^3] int32, image[(2R+1)^3,3] int8), (a,b,c) lexicographic."""
+    nn = (2 * R + 1) ** 3
+    ids = np.empty(nn, dtype=np.int32)
+    img = np.empty((nn, 3), dtype=np.int8)
+    _load().nfo_neighbors(cpd, R, int(cellid), ids.ctypes.data, img.ctypes.data)
+    return ids, img
+
+
+def pair_count(offsets: np.ndarray, cpd: int, R: int) -> int:
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    return int(_load().nfo_pair_count(offsets.ctypes.data, cpd, R))
+
+
+def accel(pos, cpd: int, R: int, eps_p: float, box: float = 1.0, gm: float | None = None,
+          sink_cells=None, nthreads: int = 0):
+    """Near-field accelerations by the definition.  -> (acc[N,3] float64, pairs evaluated).
+
+    ``sink_cells``: optional int32 array of cell ids; only particles in those cells are
+    evaluated (the rest of ``acc`` stays 0).  ``gm`` defaults to 1/N."""
+    p = _f32pos(pos)
+    N = p.shape[0]
+    if gm is None:
+        gm = 1.0 / max(N, 1)
+    acc = np.zeros((N, 3), dtype=np.float64)
+    if sink_cells is None:
+        sc_ptr, nsc = None, 0
+    else:
+        sc = np.ascontiguousarray(sink_cells, dtype=np.int32)
+        sc_ptr, nsc = sc.ctypes.data, sc.shape[0]
+    pairs = _load().nfo_accel(p.ctypes.data, N, cpd, R, float(eps_p), float(box), float(gm),
+                              sc_ptr, nsc, acc.ctypes.data, int(nthreads))
+    if pairs < 0:
+        raise ValueError("nfo_accel: bad arguments or non-finite position")
+    return acc, int(pairs)
