@@ -1,0 +1,172 @@
+/*
+ * nearfield.h -- C ABI of libnearfield_b200.so: the Abacus near-field force on one B200.
+ *
+ * What the library computes (reference: /root/reference/PAPER.md, arXiv 2110.11392):
+ *   "every cell interacting with itself and its 124 nearest neighbor cells (for near-field
+ *   radius R=2) using open boundary conditions and Newtonian gravity, or a softened form
+ *   thereof" (sec. 3.4.1) on a periodic grid of CPD^3 cells, with
+ *   the spline softening law of Eq. 3 and eps_s = 2.16 eps_p:
+ *
+ *       a_i = gm * sum_{j in the (2R+1)^3 cells around cell(i), j != i} F(x_j - x_i + image)
+ *       F(r) = [10 - 15u + 6u^2] r / eps_s^3   (u = |r|/eps_s < 1),   r/|r|^3 otherwise.
+ *
+ *   The periodic image is the whole-cell shift of the CELL PAIR, not the
+ *   particle minimum image.  Steps run by nf_accel, all in CUDA kernels for sm_100a
+ *   (DESIGN.md "The path"): A1 cell key + histogram, A2 exclusive scan, A3 stable scatter into
+ *   grid order with cell-relative float32 offsets, A4 pencil scheduler
+ *   (PAPER.md:226-236), A5 pencil-on-pencil interaction kernel, A6 un-permute to input order.
+ *
+ * Conventions
+ *   - Plain pointers and sizes only.  "d_" = device pointer on the context's device,
+ *     "h_" = host pointer.  float = IEEE binary32.  Positions/accelerations are N x 3, xyz
+ *     interleaved, contiguous (three floats per particle).
+ *   - The caller owns every buffer it passes in.  The library never frees, reallocates or
+ *     writes d_pos / h_pos.  The context owns all scratch (grow-only).
+ *   - All device work of nf_accel is enqueued on `cuda_stream` (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream); the call returns without synchronising.
+ *     One context = one call in flight.
+ *   - Every function returns an nf_status and never throws or aborts; nf_last_error gives
+ *     the text of the last failure on that context.
+ *   - There is no CPU fallback: without a CUDA device nf_create fails with NF_ECUDA.
+ */
+#ifndef NEARFIELD_B200_H
+#define NEARFIELD_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nf_ctx nf_ctx; /* opaque; created by nf_create, freed by nf_destroy */
+
+typedef enum {
+    NF_OK = 0,
+    NF_EINVAL = 1, /* bad argument (see each function) */
+    NF_ECUDA = 2,  /* a CUDA runtime call failed (text in nf_last_error) */
+    NF_ENOMEM = 3, /* device or host allocation failed */
+    NF_EPOS = 4    /* a position was NaN or infinite (reported by nf_sync) */
+} nf_status;
+
+#define NF_MAX_R 4          /* compiled maximum near-field radius */
+#define NF_N_STAGES 8       /* entries of nf_stage_ms */
+
+/*
+ * nf_create -- make a context for a grid of cpd^3 cells of a periodic box of side `box`,
+ * near-field radius R cells and Plummer-equivalent softening length
+ * eps_plummer (same length unit as box and positions; converted internally to the spline
+ * length eps_s = 2.16 eps_plummer).  Uses the current CUDA device.
+ * NF_EINVAL: out == NULL, R < 1, R > NF_MAX_R, cpd < 2R+1, cpd^3 >= 2^31, eps_plummer <= 0
+ * or not finite, box <= 0 or not finite.  NF_ECUDA: no usable device.
+ */
+nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer, double box);
+
+/* nf_destroy -- synchronise the context's last stream, free all scratch.  NULL is NF_OK. */
+nf_status nf_destroy(nf_ctx *ctx);
+
+/*
+ * nf_set_gm -- G*m of the (equal-mass) particles, the factor in a_i = gm * sum F
+ * (kernel has no mass; equal masses 1/N with G=1 in BASELINE.json).
+ * gm <= 0 (the default) means "1/N of each call".  NF_EINVAL: ctx NULL or gm not finite.
+ */
+nf_status nf_set_gm(nf_ctx *ctx, double gm);
+
+/*
+ * nf_accel -- near-field accelerations of N particles.
+ *   d_pos  [in]  device, N*3 floats, positions; any finite value is wrapped periodically
+ *                into [0, box) by the cell index (half-open cells, floor).
+ *   d_acc  [out] device, N*3 floats, a_i in (length unit)/time^2 for gm in those units,
+ *                in INPUT order.  Must not overlap d_pos.
+ *   cuda_stream  cudaStream_t as void*.
+ * Enqueues A1..A6 on the stream and returns.  N == 0 is NF_OK and does nothing.
+ * NF_EINVAL: ctx/d_pos/d_acc NULL (with N > 0), N < 0, N + cpd^3 >= 2^31 - 8.
+ * NF_ENOMEM / NF_ECUDA: scratch allocation or a launch failed.
+ * A NaN/Inf position does not fail this call: the particle is binned into cell 0, the
+ * result is unspecified, and the next nf_sync returns NF_EPOS.
+ */
+nf_status nf_accel(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc, void *cuda_stream);
+
+/*
+ * nf_accel_host -- the same through HOST buffers: copies h_pos to the device, runs
+ * nf_accel, copies the result back into h_acc and synchronises (this is the end-to-end
+ * call bench.py times; pinned host memory makes the copies asynchronous DMA).
+ * Errors as nf_accel, plus NF_EPOS for a non-finite position.
+ */
+nf_status nf_accel_host(nf_ctx *ctx, const float *h_pos, int64_t N, float *h_acc);
+
+/*
+ * nf_sync -- wait for the last nf_accel on this context and report deferred errors:
+ * NF_EPOS if it saw a non-finite position, NF_ECUDA if the stream failed.
+ */
+nf_status nf_sync(nf_ctx *ctx);
+
+/* nf_last_error -- text of the last failure ("" if none); owned by ctx (or static if ctx
+ * is NULL), valid until the next call on ctx. */
+const char *nf_last_error(const nf_ctx *ctx);
+
+/*
+ * nf_set_option -- tuning / instrumentation knobs (all have working defaults):
+ *   "stage_timing" (0/1)  record CUDA events between stages for nf_stage_ms
+ *   "kahan"        (0/1)  compensated fold of per-segment partial sums (default 1)
+ *   "heavy_first"  (0/1)  order sink blocks by descending estimated cost (default 1)
+ * NF_EINVAL: unknown name or value out of range.
+ */
+nf_status nf_set_option(nf_ctx *ctx, const char *name, double value);
+
+/*
+ * nf_stage_ms -- device time of each stage of the last nf_accel, in milliseconds
+ * (needs option "stage_timing" = 1; synchronises):
+ *   [0] A1 key+histogram  [1] A2 scans  [2] A3 scatter+rank+gather  [3] A4 scheduler
+ *   [4] A5 interaction kernel (with fused A6 un-permute)  [5] whole call  [6],[7] reserved
+ */
+nf_status nf_stage_ms(nf_ctx *ctx, float *h_ms /* NF_N_STAGES */);
+
+/* ---- exports for the bit-exact checks and for throughput accounting ------------------- */
+
+/*
+ * nf_debug_cells -- borrowed device pointers to the grid-order structures of the last
+ * nf_accel (valid until the next nf_accel / nf_destroy on ctx; synchronise first):
+ *   *d_offsets  uint32[cpd^3 + 1]  first grid-order slot of each cell, key = (cx*cpd+cy)*cpd+cz
+ *   *d_perm     uint32[N]          input index of the particle in each grid-order slot;
+ *                                  ascending input index within a cell (stable).
+ *   *d_sorted   float[4][Npad]     four planes (x, y, z offsets from the cell centre in CELL
+ *                                  units, then the cell key as uint32) in PADDED slot order;
+ *   *d_poffsets uint32[cpd^3 + 1]  first padded slot of each cell (cells padded to even size)
+ * Any out-pointer may be NULL.
+ */
+nf_status nf_debug_cells(nf_ctx *ctx, const uint32_t **d_offsets, const uint32_t **d_perm,
+                         const float **d_sorted, const uint32_t **d_poffsets, int64_t *h_npad);
+
+/* nf_debug_read -- copy `bytes` from a device pointer handed out by nf_debug_cells to host
+ * memory (synchronous).  NF_EINVAL on NULL arguments. */
+nf_status nf_debug_read(nf_ctx *ctx, const void *d_src, void *h_dst, uint64_t bytes);
+
+/*
+ * nf_debug_neighbors -- the neighbour list the interaction kernel's segment enumerator
+ * visits for sink cell `cell`: (2R+1)^3 entries in (a,b,c) lexicographic order,
+ * h_ids[n] = neighbour cell key, h_image[3n..3n+2] = periodic image counts in {-1,0,1}
+ * (PAPER.md:218, :232).  Produced on the device by the same code the kernel runs.
+ */
+nf_status nf_debug_neighbors(nf_ctx *ctx, int cell, int32_t *h_ids, int8_t *h_image);
+
+/*
+ * nf_interaction_count -- pairs (sink, source), source != sink, of the last nf_accel:
+ * sum_c n_c * sum_{c' in N(c)} n_c'  -  N, counted on the device from the cell offsets.
+ * Padding and masked lanes are not work.  Synchronises.
+ */
+nf_status nf_interaction_count(nf_ctx *ctx, int64_t *h_pairs);
+
+/*
+ * nf_probe_pipes -- microbenchmarks that give the roofline denominators on this device:
+ *   h_out[0] FP32 FMA-pipe lane-operations per second, scalar FFMA stream
+ *   h_out[1] the same for packed fma.rn.f32x2 (two lanes per thread-instruction)
+ *   h_out[2] MUFU.RSQ lane-operations per second
+ *   h_out[3] SM count   h_out[4] SM clock (MHz) reported by the runtime
+ * Runs on the current device, synchronises.  NF_EINVAL: h_out NULL.
+ */
+nf_status nf_probe_pipes(double *h_out /* 5 */);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NEARFIELD_B200_H */

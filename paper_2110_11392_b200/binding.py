@@ -1,0 +1,206 @@
+"""Thin ctypes binding of ``include/nearfield.h`` -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``libnearfield_b200.so``; there is no CPU
+fallback.  If the library is missing this module raises at import (build it with
+``python -m paper_2110_11392_b200.build``).  PyTorch supplies device memory and streams.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+NF_OK, NF_EINVAL, NF_ECUDA, NF_ENOMEM, NF_EPOS = 0, 1, 2, 3, 4
+_STATUS = {0: "NF_OK", 1: "NF_EINVAL", 2: "NF_ECUDA", 3: "NF_ENOMEM", 4: "NF_EPOS"}
+NF_N_STAGES = 8
+STAGE_NAMES = ["A1_key_hist", "A2_scan", "A3_scatter_rank_gather", "A4_scheduler",
+               "A5_interact_A6_unpermute", "total", "reserved6", "reserved7"]
+
+# every symbol include/nearfield.h declares
+SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", "nf_sync",
+           "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
+           "nf_interaction_count", "nf_probe_pipes", "nf_debug_read"]
+
+
+class NearFieldError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libnearfield_b200.so")
+
+
+def load_library() -> ctypes.CDLL:
+    path = lib_path()
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is not built (python -m paper_2110_11392_b200.build); "
+                          "there is no CPU fallback")
+    L = ctypes.CDLL(path)
+    vp, i64, i32, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
+    L.nf_create.restype = i32
+    L.nf_create.argtypes = [ctypes.POINTER(vp), i32, i32, dbl, dbl]
+    L.nf_destroy.restype = i32
+    L.nf_destroy.argtypes = [vp]
+    L.nf_set_gm.restype = i32
+    L.nf_set_gm.argtypes = [vp, dbl]
+    L.nf_accel.restype = i32
+    L.nf_accel.argtypes = [vp, vp, i64, vp, vp]
+    L.nf_accel_host.restype = i32
+    L.nf_accel_host.argtypes = [vp, vp, i64, vp]
+    L.nf_sync.restype = i32
+    L.nf_sync.argtypes = [vp]
+    L.nf_last_error.restype = ctypes.c_char_p
+    L.nf_last_error.argtypes = [vp]
+    L.nf_set_option.restype = i32
+    L.nf_set_option.argtypes = [vp, ctypes.c_char_p, dbl]
+    L.nf_stage_ms.restype = i32
+    L.nf_stage_ms.argtypes = [vp, vp]
+    L.nf_debug_cells.restype = i32
+    L.nf_debug_cells.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp),
+                                 ctypes.POINTER(vp), ctypes.POINTER(i64)]
+    L.nf_debug_neighbors.restype = i32
+    L.nf_debug_neighbors.argtypes = [vp, i32, vp, vp]
+    L.nf_interaction_count.restype = i32
+    L.nf_interaction_count.argtypes = [vp, ctypes.POINTER(i64)]
+    L.nf_debug_read.restype = i32
+    L.nf_debug_read.argtypes = [vp, vp, vp, ctypes.c_uint64]
+    L.nf_probe_pipes.restype = i32
+    L.nf_probe_pipes.argtypes = [vp]
+    return L
+
+
+_L = load_library()
+
+
+def probe_pipes() -> dict:
+    """nf_probe_pipes: measured FP32-FMA / packed-FMA / MUFU.RSQ lane rates of the device."""
+    out = (ctypes.c_double * 5)()
+    rc = _L.nf_probe_pipes(out)
+    if rc != NF_OK:
+        raise NearFieldError(rc, "nf_probe_pipes")
+    return {"ffma_lane_ops_per_s": out[0], "ffma2_lane_ops_per_s": out[1], "mufu_rsq_lane_ops_per_s": out[2],
+            "sm_count": int(out[3]), "sm_clock_mhz": out[4]}
+
+
+class NearField:
+    """nf_create / nf_accel / nf_destroy with torch tensors (or host numpy arrays) as buffers."""
+
+    def __init__(self, cpd: int, R: int, eps_plummer: float, box: float = 1.0):
+        self._h = ctypes.c_void_p()
+        rc = _L.nf_create(ctypes.byref(self._h), int(cpd), int(R), float(eps_plummer), float(box))
+        if rc != NF_OK:
+            raise NearFieldError(rc, _L.nf_last_error(None).decode())
+        self.cpd, self.R, self.eps_plummer, self.box = int(cpd), int(R), float(eps_plummer), float(box)
+        self._N = 0
+
+    # -- helpers
+    def _check(self, rc: int):
+        if rc != NF_OK:
+            raise NearFieldError(rc, _L.nf_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            _L.nf_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # -- the path
+    def set_gm(self, gm: float):
+        self._check(_L.nf_set_gm(self._h, float(gm)))
+
+    def set_option(self, name: str, value: float):
+        self._check(_L.nf_set_option(self._h, name.encode(), float(value)))
+
+    def accel(self, pos, acc=None, stream=None):
+        """pos: CUDA float32 tensor [N,3] (contiguous).  Returns acc [N,3] on the same device.
+        Enqueued on ``stream`` (default: torch's current stream); not synchronised."""
+        import torch
+        if not (pos.is_cuda and pos.dtype == torch.float32 and pos.is_contiguous() and pos.dim() == 2 and pos.shape[1] == 3):
+            raise ValueError("pos must be a contiguous CUDA float32 tensor of shape [N,3]")
+        N = pos.shape[0]
+        if acc is None:
+            acc = torch.empty_like(pos)
+        elif not (acc.is_cuda and acc.dtype == torch.float32 and acc.is_contiguous() and acc.shape == pos.shape):
+            raise ValueError("acc must match pos")
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        self._N = N
+        self._check(_L.nf_accel(self._h, pos.data_ptr() if N else None, N, acc.data_ptr() if N else None,
+                                ctypes.c_void_p(st.cuda_stream)))
+        return acc
+
+    def accel_ptr(self, d_pos: int, N: int, d_acc: int, cuda_stream: int = 0):
+        """raw-pointer form of nf_accel (used by tests of the error paths)."""
+        self._N = N
+        self._check(_L.nf_accel(self._h, ctypes.c_void_p(d_pos), int(N), ctypes.c_void_p(d_acc), ctypes.c_void_p(cuda_stream)))
+
+    def accel_host(self, h_pos: np.ndarray, h_acc: np.ndarray | None = None) -> np.ndarray:
+        """nf_accel_host: host float32 [N,3] in, host float32 [N,3] out; synchronous."""
+        h_pos = np.ascontiguousarray(h_pos, dtype=np.float32)
+        if h_acc is None:
+            h_acc = np.empty_like(h_pos)
+        self._N = h_pos.shape[0]
+        self._check(_L.nf_accel_host(self._h, h_pos.ctypes.data, h_pos.shape[0], h_acc.ctypes.data))
+        return h_acc
+
+    def accel_host_ptr(self, h_pos_ptr: int, N: int, h_acc_ptr: int):
+        self._N = N
+        self._check(_L.nf_accel_host(self._h, ctypes.c_void_p(h_pos_ptr), int(N), ctypes.c_void_p(h_acc_ptr)))
+
+    def sync(self):
+        self._check(_L.nf_sync(self._h))
+
+    def stage_ms(self) -> dict:
+        buf = (ctypes.c_float * NF_N_STAGES)()
+        self._check(_L.nf_stage_ms(self._h, buf))
+        return {STAGE_NAMES[i]: float(buf[i]) for i in range(6)}
+
+    def interaction_count(self) -> int:
+        v = ctypes.c_int64()
+        self._check(_L.nf_interaction_count(self._h, ctypes.byref(v)))
+        return int(v.value)
+
+    def debug_neighbors(self, cell: int):
+        nn = (2 * self.R + 1) ** 3
+        ids = np.empty(nn, dtype=np.int32)
+        img = np.empty((nn, 3), dtype=np.int8)
+        self._check(_L.nf_debug_neighbors(self._h, int(cell), ids.ctypes.data, img.ctypes.data))
+        return ids, img
+
+    def debug_cells(self):
+        """-> dict of host numpy copies: offsets[cpd^3+1], perm[N], poffsets[cpd^3+1],
+        sorted_xyz[Npad,3] (cell units), sorted_key[Npad] (high bit = padding slot)."""
+        self.sync()
+        p_off, p_perm, p_sorted, p_poff = (ctypes.c_void_p() for _ in range(4))
+        stride = ctypes.c_int64()
+        self._check(_L.nf_debug_cells(self._h, ctypes.byref(p_off), ctypes.byref(p_perm), ctypes.byref(p_sorted),
+                                      ctypes.byref(p_poff), ctypes.byref(stride)))
+        ncell = self.cpd ** 3
+
+        def d2h(ptr, count, dtype):
+            out = np.empty(count, dtype=dtype)
+            if count:
+                self._check(_L.nf_debug_read(self._h, ctypes.c_void_p(ptr), out.ctypes.data, out.nbytes))
+            return out
+
+        offsets = d2h(p_off.value, ncell + 1, np.uint32)
+        poff = d2h(p_poff.value, ncell + 1, np.uint32)
+        perm = d2h(p_perm.value, self._N, np.uint32)
+        npad, st = int(poff[-1]), int(stride.value)
+        planes = [d2h(p_sorted.value + 4 * st * k, npad, np.float32 if k < 3 else np.uint32) for k in range(4)]
+        return {"offsets": offsets, "perm": perm, "poffsets": poff,
+                "sorted_xyz": np.stack(planes[:3], -1), "sorted_key": planes[3]}

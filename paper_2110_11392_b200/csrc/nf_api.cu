@@ -1,0 +1,267 @@
+// nf_api.cu -- the C ABI of include/nearfield.h: argument checks, scratch management, stage
+// sequencing.  No arithmetic of the method lives here.
+#include <math.h>
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+#include "nf_common.cuh"
+
+static char g_static_err[256] = "";
+
+static void free_scratch(nf_ctx *c) {
+    void *ptrs[] = {c->d_key, c->d_arr, c->d_tmp_perm, c->d_perm_true, c->d_perm_pad, c->d_sorted, c->d_blk, c->d_blk_order};
+    for (void *p : ptrs) if (p) cudaFree(p);
+    c->d_key = c->d_arr = c->d_tmp_perm = c->d_perm_true = c->d_perm_pad = nullptr;
+    c->d_sorted = nullptr; c->d_blk = nullptr; c->d_blk_order = nullptr;
+    c->capN = c->capPad = c->capBlk = 0;
+}
+
+extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer, double box) {
+    if (!out) { snprintf(g_static_err, sizeof g_static_err, "nf_create: out is NULL"); return NF_EINVAL; }
+    *out = nullptr;
+    if (R < 1 || R > NF_MAX_R || cpd < 2 * R + 1 || !(eps_plummer > 0) || !isfinite(eps_plummer) || !(box > 0) || !isfinite(box) ||
+        (double)cpd * cpd * cpd >= 2147483648.0) {
+        snprintf(g_static_err, sizeof g_static_err, "nf_create: bad argument (cpd=%d R=%d eps=%g box=%g)", cpd, R, eps_plummer, box);
+        return NF_EINVAL;
+    }
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        snprintf(g_static_err, sizeof g_static_err, "nf_create: no CUDA device (there is no CPU fallback)");
+        return NF_ECUDA;
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major < 10) {
+        snprintf(g_static_err, sizeof g_static_err, "nf_create: device is not sm_100 class (compute %d.%d)", prop.major, prop.minor);
+        return NF_ECUDA;
+    }
+    nf_ctx *c = new (std::nothrow) nf_ctx;
+    if (!c) return NF_ENOMEM;
+    memset(c, 0, sizeof *c);
+    c->device = dev; c->cpd = cpd; c->R = R; c->eps_p = eps_plummer; c->box = box; c->gm = 0.0;
+    c->sm_count = prop.multiProcessorCount;
+    c->ncell = (int64_t)cpd * cpd * cpd; c->ncol = (int64_t)cpd * cpd;
+    c->opt_kahan = 1; c->opt_heavy_first = 1; c->opt_stage_timing = 0;
+    NfParams &p = c->prm;
+    p.cpd = cpd; p.R = R; p.ncell = (int)c->ncell; p.ncol = (int)c->ncol;
+    p.scale = (double)cpd / box;
+    const double e = NF_SPLINE_PER_PLUMMER * eps_plummer * p.scale;   // eps_s in cell units
+    p.c0 = (float)(10.0 / (e * e * e));
+    p.c1 = (float)(-15.0 / (e * e * e * e));
+    p.c2 = (float)(6.0 / (e * e * e * e * e));
+    int nc = (int)ceil(e);
+    if (nc < 1) nc = 1;
+    if (nc > R) nc = R;
+    p.near_cheb = nc;
+    p.kahan = 1;
+    nf_status rc = NF_OK;
+    auto fail = [&](nf_status s) { snprintf(g_static_err, sizeof g_static_err, "%s", c->err); nf_destroy(c); return s; };
+#define TRY_ALLOC(ptr, bytes)                                                                  \
+    if (cudaMalloc((void **)&(ptr), (bytes)) != cudaSuccess) {                                  \
+        cudaGetLastError(); snprintf(c->err, sizeof c->err, "nf_create: cudaMalloc(%zu) failed", (size_t)(bytes)); \
+        return fail(NF_ENOMEM);                                                                 \
+    }
+    const size_t nscan = (size_t)((c->ncell + 2047) / 2048 + 8);
+    TRY_ALLOC(c->d_counts, (size_t)(c->ncell + 1) * 4);
+    TRY_ALLOC(c->d_offsets, (size_t)(c->ncell + 1) * 4);
+    TRY_ALLOC(c->d_poff, (size_t)(c->ncell + 1) * 4);
+    TRY_ALLOC(c->d_scan_blk, nscan * 8);
+    TRY_ALLOC(c->d_col_nblk, (size_t)(c->ncol + 1) * 4);
+    TRY_ALLOC(c->d_col_base, (size_t)(c->ncol + 1) * 4);
+    TRY_ALLOC(c->d_ctrl, 128 * 4);
+    TRY_ALLOC(c->d_pairs, 8);
+    TRY_ALLOC(c->d_nbr, (size_t)4 * 729 * 4);
+#undef TRY_ALLOC
+    for (int i = 0; i < 8; ++i)
+        if (cudaEventCreate(&c->ev[i]) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaEventCreate failed"); return fail(NF_ECUDA); }
+    if (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaStreamCreate failed"); return fail(NF_ECUDA); }
+    rc = nf_interact_setup(c);
+    if (rc != NF_OK) return fail(rc);
+    *out = c;
+    return NF_OK;
+}
+
+extern "C" nf_status nf_destroy(nf_ctx *c) {
+    if (!c) return NF_OK;
+    cudaSetDevice(c->device);
+    cudaDeviceSynchronize();
+    free_scratch(c);
+    void *ptrs[] = {c->d_counts, c->d_offsets, c->d_poff, c->d_scan_blk, c->d_col_nblk, c->d_col_base, c->d_ctrl, c->d_pairs, c->d_nbr, c->d_pos_buf, c->d_acc_buf};
+    for (void *p : ptrs) if (p) cudaFree(p);
+    for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    if (c->own_stream) cudaStreamDestroy(c->own_stream);
+    cudaGetLastError();
+    delete c;
+    return NF_OK;
+}
+
+extern "C" const char *nf_last_error(const nf_ctx *c) { return c ? c->err : g_static_err; }
+
+extern "C" nf_status nf_set_gm(nf_ctx *c, double gm) {
+    if (!c || !isfinite(gm)) return NF_EINVAL;
+    c->gm = gm;
+    return NF_OK;
+}
+
+extern "C" nf_status nf_set_option(nf_ctx *c, const char *name, double v) {
+    if (!c || !name) return NF_EINVAL;
+    const int iv = (int)v;
+    if (v != 0.0 && v != 1.0) { snprintf(c->err, sizeof c->err, "nf_set_option(%s): value must be 0 or 1", name); return NF_EINVAL; }
+    if (!strcmp(name, "stage_timing")) c->opt_stage_timing = iv;
+    else if (!strcmp(name, "kahan")) c->opt_kahan = iv;
+    else if (!strcmp(name, "heavy_first")) c->opt_heavy_first = iv;
+    else { snprintf(c->err, sizeof c->err, "nf_set_option: unknown option '%s'", name); return NF_EINVAL; }
+    return NF_OK;
+}
+
+static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
+    if (N <= c->capN) return NF_OK;
+    cudaStreamSynchronize(c->last_stream);
+    free_scratch(c);
+    const int64_t capPad = ((N + c->ncell + 8 + 3) / 4) * 4 + 8;
+    const int64_t capBlk = capPad / NF_BS + c->ncol + 8;
+    cudaError_t e = cudaSuccess;
+    auto A = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
+    A((void **)&c->d_key, (size_t)N * 4);
+    A((void **)&c->d_arr, (size_t)N * 4);
+    A((void **)&c->d_tmp_perm, (size_t)capPad * 4);
+    A((void **)&c->d_perm_true, (size_t)N * 4);
+    A((void **)&c->d_perm_pad, (size_t)capPad * 4);
+    A((void **)&c->d_sorted, (size_t)capPad * 16);
+    A((void **)&c->d_blk, (size_t)capBlk * sizeof(NfBlockDesc));
+    A((void **)&c->d_blk_order, (size_t)capBlk * 4);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        free_scratch(c);
+        snprintf(c->err, sizeof c->err, "nf_accel: scratch allocation for N=%lld failed: %s", (long long)N, cudaGetErrorString(e));
+        return NF_ENOMEM;
+    }
+    c->capN = N; c->capPad = capPad; c->capBlk = capBlk;
+    return NF_OK;
+}
+
+extern "C" nf_status nf_accel(nf_ctx *c, const float *d_pos, int64_t N, float *d_acc, void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N < 0 || (N > 0 && (!d_pos || !d_acc)) || (double)N + (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_accel: bad argument (N=%lld)", (long long)N);
+        return NF_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (N == 0) return NF_OK;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    nf_status rc = ensure_scratch(c, N);
+    if (rc != NF_OK) return rc;
+    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    if (c->opt_stage_timing) cudaEventRecord(c->ev[6], st);
+    rc = nf_run_binner(c, d_pos, N, st);
+    if (rc != NF_OK) return rc;
+    rc = nf_run_scheduler(c, N, st);
+    if (rc != NF_OK) return rc;
+    if (c->opt_stage_timing) cudaEventRecord(c->ev[4], st);
+    const double gm = c->gm > 0 ? c->gm : 1.0 / (double)N;
+    const double cellsz = c->box / (double)c->cpd;
+    const float kfac = (float)(gm / (cellsz * cellsz));
+    rc = nf_run_interact(c, N, d_acc, kfac, st);
+    if (rc != NF_OK) return rc;
+    if (c->opt_stage_timing) { cudaEventRecord(c->ev[5], st); cudaEventRecord(c->ev[7], st); }
+    return NF_OK;
+}
+
+extern "C" nf_status nf_sync(nf_ctx *c) {
+    if (!c) return NF_EINVAL;
+    if (!c->have_last) return NF_OK;
+    NF_CUDA_OK(c, cudaStreamSynchronize(c->last_stream));
+    uint32_t ctrl[4];
+    NF_CUDA_OK(c, cudaMemcpy(ctrl, c->d_ctrl, sizeof ctrl, cudaMemcpyDeviceToHost));
+    if (ctrl[2]) { snprintf(c->err, sizeof c->err, "nf_accel: a position was NaN or infinite"); return NF_EPOS; }
+    return NF_OK;
+}
+
+extern "C" nf_status nf_accel_host(nf_ctx *c, const float *h_pos, int64_t N, float *h_acc) {
+    if (!c) return NF_EINVAL;
+    if (N < 0 || (N > 0 && (!h_pos || !h_acc))) { snprintf(c->err, sizeof c->err, "nf_accel_host: bad argument"); return NF_EINVAL; }
+    if (N == 0) return NF_OK;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    if (N > c->capHost) {
+        if (c->d_pos_buf) cudaFree(c->d_pos_buf);
+        if (c->d_acc_buf) cudaFree(c->d_acc_buf);
+        c->d_pos_buf = c->d_acc_buf = nullptr; c->capHost = 0;
+        NF_CUDA_OK(c, cudaMalloc((void **)&c->d_pos_buf, (size_t)N * 12));
+        NF_CUDA_OK(c, cudaMalloc((void **)&c->d_acc_buf, (size_t)N * 12));
+        c->capHost = N;
+    }
+    cudaStream_t st = c->own_stream;
+    NF_CUDA_OK(c, cudaMemcpyAsync(c->d_pos_buf, h_pos, (size_t)N * 12, cudaMemcpyHostToDevice, st));
+    nf_status rc = nf_accel(c, c->d_pos_buf, N, c->d_acc_buf, (void *)st);
+    if (rc != NF_OK) return rc;
+    NF_CUDA_OK(c, cudaMemcpyAsync(h_acc, c->d_acc_buf, (size_t)N * 12, cudaMemcpyDeviceToHost, st));
+    return nf_sync(c);
+}
+
+extern "C" nf_status nf_stage_ms(nf_ctx *c, float *h_ms) {
+    if (!c || !h_ms) return NF_EINVAL;
+    for (int i = 0; i < NF_N_STAGES; ++i) h_ms[i] = 0.f;
+    if (!c->have_last || !c->opt_stage_timing) { snprintf(c->err, sizeof c->err, "nf_stage_ms: enable option stage_timing and call nf_accel first"); return NF_EINVAL; }
+    NF_CUDA_OK(c, cudaStreamSynchronize(c->last_stream));
+    NF_CUDA_OK(c, cudaEventElapsedTime(&h_ms[0], c->ev[0], c->ev[1]));
+    NF_CUDA_OK(c, cudaEventElapsedTime(&h_ms[1], c->ev[1], c->ev[2]));
+    NF_CUDA_OK(c, cudaEventElapsedTime(&h_ms[2], c->ev[2], c->ev[3]));
+    NF_CUDA_OK(c, cudaEventElapsedTime(&h_ms[3], c->ev[3], c->ev[4]));
+    NF_CUDA_OK(c, cudaEventElapsedTime(&h_ms[4], c->ev[4], c->ev[5]));
+    NF_CUDA_OK(c, cudaEventElapsedTime(&h_ms[5], c->ev[6], c->ev[7]));
+    return NF_OK;
+}
+
+extern "C" nf_status nf_debug_cells(nf_ctx *c, const uint32_t **d_offsets, const uint32_t **d_perm, const float **d_sorted,
+                                    const uint32_t **d_poffsets, int64_t *h_npad) {
+    if (!c) return NF_EINVAL;
+    if (!c->have_last) { snprintf(c->err, sizeof c->err, "nf_debug_cells: no nf_accel call yet"); return NF_EINVAL; }
+    if (d_offsets) *d_offsets = c->d_offsets;
+    if (d_perm) *d_perm = c->d_perm_true;
+    if (d_sorted) *d_sorted = c->d_sorted;
+    if (d_poffsets) *d_poffsets = c->d_poff;
+    if (h_npad) *h_npad = c->capPad;   // plane stride of d_sorted
+    return NF_OK;
+}
+
+extern "C" nf_status nf_debug_read(nf_ctx *c, const void *d_src, void *h_dst, uint64_t bytes) {
+    if (!c || !d_src || !h_dst) return NF_EINVAL;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    if (c->have_last) NF_CUDA_OK(c, cudaStreamSynchronize(c->last_stream));
+    NF_CUDA_OK(c, cudaMemcpy(h_dst, d_src, (size_t)bytes, cudaMemcpyDeviceToHost));
+    return NF_OK;
+}
+
+extern "C" nf_status nf_debug_neighbors(nf_ctx *c, int cell, int32_t *h_ids, int8_t *h_image) {
+    if (!c || !h_ids || !h_image || cell < 0 || cell >= c->ncell) return NF_EINVAL;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    const int w = 2 * c->R + 1, nn = w * w * w;
+    nf_status rc = nf_run_neighbors(c, cell, c->own_stream);
+    if (rc != NF_OK) return rc;
+    int32_t *tmp = (int32_t *)malloc((size_t)nn * 4 * sizeof(int32_t));
+    if (!tmp) return NF_ENOMEM;
+    cudaError_t e = cudaMemcpyAsync(tmp, c->d_nbr, (size_t)nn * 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, c->own_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->own_stream);
+    if (e != cudaSuccess) { free(tmp); snprintf(c->err, sizeof c->err, "nf_debug_neighbors: %s", cudaGetErrorString(e)); return NF_ECUDA; }
+    for (int n = 0; n < nn; ++n) {
+        h_ids[n] = tmp[n];
+        for (int k = 0; k < 3; ++k) h_image[3 * n + k] = (int8_t)tmp[nn + 3 * n + k];
+    }
+    free(tmp);
+    return NF_OK;
+}
+
+extern "C" nf_status nf_interaction_count(nf_ctx *c, int64_t *h_pairs) {
+    if (!c || !h_pairs) return NF_EINVAL;
+    if (!c->have_last) { snprintf(c->err, sizeof c->err, "nf_interaction_count: no nf_accel call yet"); return NF_EINVAL; }
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    NF_CUDA_OK(c, cudaStreamSynchronize(c->last_stream));
+    nf_status rc = nf_run_paircount(c, c->own_stream);
+    if (rc != NF_OK) return rc;
+    unsigned long long v = 0;
+    NF_CUDA_OK(c, cudaMemcpyAsync(&v, c->d_pairs, 8, cudaMemcpyDeviceToHost, c->own_stream));
+    NF_CUDA_OK(c, cudaStreamSynchronize(c->own_stream));
+    *h_pairs = (int64_t)v - c->lastN;
+    return NF_OK;
+}

@@ -1,0 +1,246 @@
+// nf_binner.cu -- steps A1..A3 of the path: counting-sort cell binner.
+//
+// PAPER.md:72  "Particles and other properties are stored in grid order, indexed by slab and by
+//              cell";  PAPER.md:264 positions are float32 offsets from cell centres;
+//              PAPER.md:399 per-cell offset + count.  The paper keeps grid order incrementally
+//              (insert list + merge slabs); for a device-resident particle
+//              set this build replaces that with a full counting sort per call.
+//
+//   A1  k_key_hist      cell key per particle (double arithmetic, half-open cells, periodic
+//                       wrap) + histogram; the atomic's return value is kept as arrival rank
+//   A2  scan            exclusive scan of the counts -> true offsets and padded offsets
+//                       (each cell padded to an even slot count) in one 64-bit scan
+//   A3  k_scatter       particle index -> its cell's slot range (arrival order)
+//       k_rank_gather   within-cell rank by ascending input index (=> stable, deterministic),
+//                       gather of the positions, cell-relative float32 offsets in CELL units,
+//                       SoA planes x | y | z | key, plus both permutations
+#include "nf_common.cuh"
+
+// ------------------------------------------------------------------------------ A1
+__device__ __forceinline__ int nf_axis_cell(float x, double scale, int cpd, int &bad) {
+    double xd = (double)x;
+    if (!isfinite(xd)) { bad = 1; return 0; }
+    double t = xd * scale;
+    double I = floor(t);
+    if (I >= 0.0 && I < (double)cpd) return (int)I;
+    double m = fmod(I, (double)cpd);      // exact
+    if (m < 0.0) m += (double)cpd;
+    return (int)m;
+}
+
+__global__ void __launch_bounds__(256) k_key_hist(const float *__restrict__ pos, uint32_t N, double scale, int cpd,
+                                                  uint32_t *__restrict__ key, uint32_t *__restrict__ arr,
+                                                  uint32_t *__restrict__ counts, uint32_t *__restrict__ ctrl) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float *p = pos + 3ull * i;
+    int bad = 0;
+    int cx = nf_axis_cell(p[0], scale, cpd, bad);
+    int cy = nf_axis_cell(p[1], scale, cpd, bad);
+    int cz = nf_axis_cell(p[2], scale, cpd, bad);
+    uint32_t k = bad ? 0u : (uint32_t)((cx * cpd + cy) * cpd + cz);
+    if (bad) ctrl[2] = 1u;
+    key[i] = k;
+    arr[i] = atomicAdd(&counts[k], 1u);
+}
+
+// ------------------------------------------------------------------------------ A2: scan
+// Three-phase exclusive scan of 64-bit items; SCAN_TILE items per block.
+#define SCAN_THREADS 256
+#define SCAN_ITEMS 8
+#define SCAN_TILE (SCAN_THREADS * SCAN_ITEMS)
+
+__device__ __forceinline__ unsigned long long block_excl_scan(unsigned long long v, unsigned long long *total) {
+    // exclusive scan of one value per thread across the block (SCAN_THREADS threads)
+    __shared__ unsigned long long wsum[SCAN_THREADS / 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned long long inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        unsigned long long o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += o;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        unsigned long long s = (lane < SCAN_THREADS / 32) ? wsum[lane] : 0ull;
+#pragma unroll
+        for (int d = 1; d < SCAN_THREADS / 32; d <<= 1) {
+            unsigned long long o = __shfl_up_sync(0xffffffffu, s, d);
+            if (lane >= d) s += o;
+        }
+        if (lane < SCAN_THREADS / 32) wsum[lane] = s;   // inclusive over warps
+    }
+    __syncthreads();
+    unsigned long long base = (w > 0) ? wsum[w - 1] : 0ull;
+    if (total) *total = wsum[SCAN_THREADS / 32 - 1];
+    __syncthreads();
+    return base + inc - v;
+}
+
+// item c of the cell scan = (padded count << 32) | true count
+__device__ __forceinline__ unsigned long long cell_item(const uint32_t *counts, uint32_t c) {
+    uint32_t n = counts[c];
+    return ((unsigned long long)((n + 1u) & ~1u) << 32) | n;
+}
+
+template <int MODE>   // 0: cells (from counts)  1: plain uint32 input widened to 64 bit
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const uint32_t *__restrict__ in, uint32_t n,
+                                                              unsigned long long *__restrict__ blk) {
+    unsigned long long s = 0;
+    uint32_t base = blockIdx.x * SCAN_TILE;
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        uint32_t c = base + k * SCAN_THREADS + threadIdx.x;
+        if (c < n) s += (MODE == 0) ? cell_item(in, c) : (unsigned long long)in[c];
+    }
+    unsigned long long tot;
+    block_excl_scan(s, &tot);
+    if (threadIdx.x == 0) blk[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_blocks(unsigned long long *blk, uint32_t nblk) {
+    // single block: exclusive scan of the block totals in place; total appended at blk[nblk]
+    unsigned long long carry = 0;
+    for (uint32_t b0 = 0; b0 < nblk; b0 += SCAN_THREADS) {
+        uint32_t b = b0 + threadIdx.x;
+        unsigned long long v = (b < nblk) ? blk[b] : 0ull, tot;
+        unsigned long long ex = block_excl_scan(v, &tot);
+        if (b < nblk) blk[b] = carry + ex;
+        carry += tot;
+    }
+    if (threadIdx.x == 0) blk[nblk] = carry;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const uint32_t *__restrict__ in, uint32_t n,
+                                                             const unsigned long long *__restrict__ blk,
+                                                             uint32_t *__restrict__ out_lo, uint32_t *__restrict__ out_hi,
+                                                             uint32_t *__restrict__ ctrl) {
+    // thread t owns SCAN_ITEMS consecutive items (blocked arrangement) so the scan is in order
+    uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+    unsigned long long v[SCAN_ITEMS], s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        uint32_t c = base + k;
+        v[k] = (c < n) ? ((MODE == 0) ? cell_item(in, c) : (unsigned long long)in[c]) : 0ull;
+        s += v[k];
+    }
+    unsigned long long ex = block_excl_scan(s, nullptr) + blk[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        uint32_t c = base + k;
+        if (c < n) {
+            out_lo[c] = (uint32_t)ex;
+            if (MODE == 0) out_hi[c] = (uint32_t)(ex >> 32);
+        }
+        ex += v[k];
+    }
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == SCAN_THREADS - 1) {
+        // grand total at index n
+        unsigned long long tot = blk[gridDim.x];
+        out_lo[n] = (uint32_t)tot;
+        if (MODE == 0) { out_hi[n] = (uint32_t)(tot >> 32); ctrl[3] = (uint32_t)(tot >> 32); }
+        else ctrl[1] = (uint32_t)tot;
+    }
+}
+// k_scan_reduce sums items in a strided arrangement, k_scan_apply in a blocked one; both cover
+// exactly the items [blockIdx*SCAN_TILE, (blockIdx+1)*SCAN_TILE), so the block totals agree.
+
+static nf_status scan_cells(nf_ctx *ctx, cudaStream_t st) {
+    uint32_t n = (uint32_t)ctx->ncell;
+    uint32_t nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
+    k_scan_reduce<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk);
+    k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(ctx->d_scan_blk, nblk);
+    k_scan_apply<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk, ctx->d_offsets, ctx->d_poff, ctx->d_ctrl);
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
+
+nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st) {
+    // exclusive scan of n uint32 values into out[0..n]; the total also goes to ctrl[1]
+    uint32_t nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
+    k_scan_reduce<1><<<nblk, SCAN_THREADS, 0, st>>>(in, n, ctx->d_scan_blk);
+    k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(ctx->d_scan_blk, nblk);
+    k_scan_apply<1><<<nblk, SCAN_THREADS, 0, st>>>(in, n, ctx->d_scan_blk, out, nullptr, ctx->d_ctrl);
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
+
+// ------------------------------------------------------------------------------ A3
+__global__ void __launch_bounds__(256) k_scatter(uint32_t N, const uint32_t *__restrict__ key, const uint32_t *__restrict__ arr,
+                                                 const uint32_t *__restrict__ counts, const uint32_t *__restrict__ poff,
+                                                 uint32_t *__restrict__ tmp_perm, uint32_t *__restrict__ skey) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    uint32_t k = key[i], r = arr[i];
+    uint32_t slot = poff[k] + r;
+    tmp_perm[slot] = i;
+    skey[slot] = k;
+    if (r == 0) {
+        uint32_t n = counts[k];
+        if (n & 1u) skey[poff[k] + n] = k | NF_PAD_FLAG;   // the padding slot of an odd cell
+    }
+}
+
+__device__ __forceinline__ float nf_axis_offset(float x, double scale) {
+    double t = (double)x * scale;
+    return (float)(t - floor(t) - 0.5);       // offset from the cell centre, cell units, [-0.5, 0.5)
+}
+
+__global__ void __launch_bounds__(256) k_rank_gather(const float *__restrict__ pos, double scale, uint32_t cap_pad,
+                                                     const uint32_t *__restrict__ ctrl, const uint32_t *__restrict__ offsets,
+                                                     const uint32_t *__restrict__ poff, const uint32_t *__restrict__ tmp_perm,
+                                                     float *__restrict__ sorted, uint32_t *__restrict__ perm_true,
+                                                     uint32_t *__restrict__ perm_pad) {
+    uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t npad = ctrl[3];
+    float *sx = sorted, *sy = sorted + cap_pad, *sz = sorted + 2ull * cap_pad;
+    uint32_t *skey = (uint32_t *)(sorted + 3ull * cap_pad);
+    if (s >= npad) {
+        if (s < npad + 8 && s < cap_pad) {    // tail slack read by 16-byte aligned bulk copies
+            sx[s] = NF_BIG; sy[s] = 0.f; sz[s] = 0.f; skey[s] = NF_PAD_FLAG; perm_pad[s] = 0xffffffffu;
+        }
+        return;
+    }
+    uint32_t k = skey[s];
+    if (k & NF_PAD_FLAG) {
+        sx[s] = NF_BIG; sy[s] = 0.f; sz[s] = 0.f; perm_pad[s] = 0xffffffffu;
+        return;
+    }
+    const uint32_t lo = poff[k], o0 = offsets[k], n = offsets[k + 1] - o0;
+    const uint32_t me = tmp_perm[s];
+    uint32_t rank = 0;
+    for (uint32_t t = 0; t < n; ++t) rank += (tmp_perm[lo + t] < me) ? 1u : 0u;
+    const float *p = pos + 3ull * me;
+    const uint32_t dst = lo + rank;
+    sx[dst] = nf_axis_offset(p[0], scale);
+    sy[dst] = nf_axis_offset(p[1], scale);
+    sz[dst] = nf_axis_offset(p[2], scale);
+    perm_pad[dst] = me;
+    perm_true[o0 + rank] = me;
+}
+
+nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st) {
+    const uint32_t n = (uint32_t)N;
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_counts, 0, (size_t)(ctx->ncell + 1) * sizeof(uint32_t), st));
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_ctrl, 0, 16 * sizeof(uint32_t), st));
+    if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[0], st);
+    k_key_hist<<<(n + 255) / 256, 256, 0, st>>>(d_pos, n, ctx->prm.scale, ctx->cpd, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_ctrl);
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[1], st);
+    nf_status rc = scan_cells(ctx, st);
+    if (rc != NF_OK) return rc;
+    if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[2], st);
+    uint32_t *skey = (uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
+    k_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_poff, ctx->d_tmp_perm, skey);
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    // upper bound of the padded slot count: N + ncell (+8 slack), known on the host
+    uint64_t bound = (uint64_t)N + (uint64_t)ctx->ncell + 8;
+    if (bound > (uint64_t)ctx->capPad) bound = ctx->capPad;
+    k_rank_gather<<<(uint32_t)((bound + 255) / 256), 256, 0, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl,
+                                                                   ctx->d_offsets, ctx->d_poff, ctx->d_tmp_perm, ctx->d_sorted,
+                                                                   ctx->d_perm_true, ctx->d_perm_pad);
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[3], st);
+    return NF_OK;
+}

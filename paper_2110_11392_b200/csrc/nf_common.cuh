@@ -1,0 +1,101 @@
+// nf_common.cuh -- shared declarations of the CUDA near-field path (sm_100a only).
+// Not shared with oracle/ in any way.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include "../../include/nearfield.h"
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "this library is written for sm_100a (B200) only"
+#endif
+
+// ---- layout constants -------------------------------------------------------------------
+#define NF_PAD_FLAG 0x80000000u   // high bit of the cell-key plane marks a padding slot
+#define NF_BIG 1.0e18f            // x offset of padding sources (+BIG) and masked sinks (-BIG): r^-3 underflows to exactly 0
+#define NF_TAU 1.0e-30f           // addend of the first r^2 product: self pairs give f*d = c0*0 = 0, no NaN
+#define NF_SPLINE_PER_PLUMMER 2.16  // eps_s = 2.16 eps_p
+
+// interaction kernel geometry
+#define NF_NW 4                   // consumer warps per CTA (one sink per thread)
+#define NF_BS (NF_NW * 32)        // sinks per CTA work item
+#define NF_TILE 1024              // source slots per pipeline stage (per coordinate plane)
+#define NF_TABMAX 31              // source cells per segment table (32 entries = one per producer lane)
+#define NF_NSTAGE 4               // pipeline depth
+
+struct NfParams {
+    int cpd, R, ncell, ncol;
+    double scale;        // cpd / box
+    float c0, c1, c2;    // spline coefficients in cell units: 10/e^3, -15/e^4, 6/e^5, e = eps_s/cell
+    int near_cheb;       // source cells at Chebyshev distance <= near_cheb may hold r < eps_s
+    int kahan;
+};
+
+struct NfBlockDesc {     // one sink work item: <= NF_BS consecutive padded slots of one z-column
+    uint32_t col;        // cx*cpd + cy
+    uint32_t s0;         // first padded slot
+    uint32_t cnt;        // number of slots
+    uint32_t cost;       // estimated cost (sinks x sources in the z-window of the home column), saturating
+};
+
+struct nf_ctx {
+    int device, cpd, R, sm_count;
+    double eps_p, box, gm;
+    int64_t ncell, ncol;
+    NfParams prm;
+    // options
+    int opt_stage_timing, opt_kahan, opt_heavy_first;
+    // scratch (grow-only)
+    int64_t capN, capPad, capBlk;
+    uint32_t *d_key, *d_arr, *d_counts, *d_offsets, *d_poff, *d_tmp_perm, *d_perm_true, *d_perm_pad;
+    unsigned long long *d_scan_in, *d_scan_blk;
+    float *d_sorted;             // 4 planes of capPad: x, y, z (cell units), cell key (uint32 bits)
+    uint32_t *d_col_nblk, *d_col_base, *d_scan32_blk, *d_blk_order;
+    NfBlockDesc *d_blk;
+    uint32_t *d_ctrl;            // [0] work counter  [1] number of blocks  [2] bad-position flag  [3] npad
+    unsigned long long *d_pairs;
+    int32_t *d_nbr;              // debug neighbour list
+    // host staging for nf_accel_host
+    float *d_pos_buf, *d_acc_buf;
+    int64_t capHost;
+    cudaStream_t own_stream;
+    // state of the last call
+    cudaStream_t last_stream;
+    int64_t lastN;
+    int have_last;
+    cudaEvent_t ev[8];
+    char err[512];
+};
+
+#define NF_CUDA_OK(ctx, call)                                                                   \
+    do {                                                                                        \
+        cudaError_t e__ = (call);                                                               \
+        if (e__ != cudaSuccess) {                                                               \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s failed: %s (%s:%d)", #call,            \
+                     cudaGetErrorString(e__), __FILE__, __LINE__);                              \
+            return (e__ == cudaErrorMemoryAllocation) ? NF_ENOMEM : NF_ECUDA;                   \
+        }                                                                                       \
+    } while (0)
+
+// stages implemented in the other translation units
+nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st);
+nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st);
+nf_status nf_run_interact(nf_ctx *ctx, int64_t N, float *d_acc, float kfac, cudaStream_t st);
+nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st);
+nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st);
+nf_status nf_interact_setup(nf_ctx *ctx);
+nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st);
+
+// ---- device helpers shared by the kernels -------------------------------------------------
+// periodic wrap of a cell index that is at most one period out of range; image = floor(v/cpd)
+__device__ __forceinline__ int nf_wrap1(int v, int cpd, int &image) {
+    image = 0;
+    if (v < 0) { v += cpd; image = -1; }
+    else if (v >= cpd) { v -= cpd; image = 1; }
+    return v;
+}
+// non-negative modulus for any int
+__device__ __forceinline__ int nf_mod(int v, int cpd) {
+    int m = v % cpd;
+    return m < 0 ? m + cpd : m;
+}

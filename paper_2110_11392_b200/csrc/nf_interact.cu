@@ -1,0 +1,472 @@
+// nf_interact.cu -- steps A4..A6: pencil scheduler, pencil-on-pencil interaction kernel with
+// fused un-permute, plus the neighbour-list and pair-count exports.
+//
+// Paper basis: PAPER.md:226-236 (sec. 3.4.2 pencil-on-pencil; sink blocks; one sink per
+// thread in registers, sources staged in shared memory), PAPER.md:132 (Eq. 3)
+// (hand-off to 1/r^2 "with a min instead of a conditional").  What differs from the paper's
+// V100 design, and why, is in DESIGN.md "Kernel design":
+//   * sinks AND sources are z-pencils (z is the fastest cell index, so the source cells
+//     (i+a, j+b, k-R..k+R) of one (a,b) column are ONE contiguous range of the sorted planes
+//     -> one cp.async.bulk per coordinate plane per column, completed on an mbarrier);
+//   * 32 consecutive grid-order sinks per warp regardless of cell boundaries; a lane whose
+//     cell is more than R cells from the current source cell is masked by moving its sink to
+//     -NF_BIG, which makes its contribution exactly 0 (no per-interaction predicate);
+//   * two sources per thread-iteration in packed fma.rn.f32x2 / add.f32x2 / mul.f32x2, so the
+//     FMA pipe (2 cycles per packed warp-instruction) is the bound, not the issue slots;
+//   * source cells that cannot hold r < eps_s skip the spline (11 instead of 14 FMA-pipe ops);
+//   * a dedicated producer warp streams (column, z-run, chunk) segments through an
+//     NF_NSTAGE-deep full/empty mbarrier ring; persistent CTAs pull sink blocks from an
+//     atomic counter in heavy-first order;
+//   * A6 is fused: each thread writes gm/cell^2 * a straight to d_acc[perm[slot]].
+#include "nf_common.cuh"
+
+// ------------------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "NF_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra NF_DONE_%=;\n\t"
+        "bra NF_WAIT_%=;\n\t"
+        "NF_DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ float mufu_rsq(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ------------------------------------------------------------------------------ A4: scheduler
+// Sink work items: every z-column (cx,cy) is cut into blocks of consecutive PADDED grid-order
+// slots, balanced within the column ("sink particles are arranged into blocks").
+__global__ void __launch_bounds__(256) k_col_blocks(int ncol, int cpd, const uint32_t *__restrict__ poff, uint32_t *__restrict__ col_nblk) {
+    int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= ncol) return;
+    uint32_t n = poff[(col + 1) * cpd] - poff[col * cpd];
+    col_nblk[col] = (n + NF_BS - 1) / NF_BS;
+}
+
+__global__ void __launch_bounds__(128) k_fill_blocks(int ncol, int cpd, const uint32_t *__restrict__ poff, const uint32_t *__restrict__ col_nblk,
+                                                     const uint32_t *__restrict__ col_base, NfBlockDesc *__restrict__ blk, int R) {
+    int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= ncol) return;
+    const uint32_t nb = col_nblk[col];
+    if (nb == 0) return;
+    const uint32_t p0 = poff[col * cpd], n = poff[(col + 1) * cpd] - p0;
+    const uint32_t bs = (((n + nb - 1) / nb) + 31u) & ~31u;
+    const uint32_t base = col_base[col];
+    // cost estimate: sinks x (sources of the whole home column window), cheap proxy = sinks x column density x (2R+1+span)
+    for (uint32_t k = 0; k < nb; ++k) {
+        NfBlockDesc d;
+        d.col = (uint32_t)col;
+        d.s0 = p0 + k * bs;
+        uint32_t rem = (k * bs < n) ? n - k * bs : 0u;
+        d.cnt = rem < bs ? rem : bs;
+        unsigned long long c = (unsigned long long)d.cnt * (unsigned long long)n;
+        d.cost = c > 0xffffffffull ? 0xffffffffu : (uint32_t)c;
+        blk[base + k] = d;
+    }
+}
+
+// Heavy-first order: counting sort of the blocks into 64 half-octave cost buckets, descending.
+__device__ __forceinline__ int cost_bucket(uint32_t c) {
+    if (!c) return 63;
+    const int l = 31 - __clz(c);
+    const int half = l > 0 ? (int)((c >> (l - 1)) & 1u) : 0;
+    return 63 - (2 * l + half);
+}
+__global__ void __launch_bounds__(256) k_order_hist(const uint32_t *__restrict__ ctrl, const NfBlockDesc *__restrict__ blk, uint32_t *__restrict__ hist) {
+    uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ctrl[1]) return;
+    atomicAdd(&hist[cost_bucket(blk[b].cost)], 1u);
+}
+__global__ void k_order_scan(uint32_t *hist) {   // 64 buckets, one thread
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        uint32_t s = 0;
+        for (int i = 0; i < 64; ++i) { uint32_t v = hist[i]; hist[i] = s; s += v; }
+    }
+}
+__global__ void __launch_bounds__(256) k_order_fill(const uint32_t *__restrict__ ctrl, const NfBlockDesc *__restrict__ blk, uint32_t *__restrict__ hist,
+                                                    uint32_t *__restrict__ order) {
+    uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ctrl[1]) return;
+    order[atomicAdd(&hist[cost_bucket(blk[b].cost)], 1u)] = b;
+}
+__global__ void __launch_bounds__(256) k_order_identity(const uint32_t *__restrict__ ctrl, uint32_t *__restrict__ order) {
+    uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < ctrl[1]) order[b] = b;
+}
+
+nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st);
+
+nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st) {
+    const int ncol = (int)ctx->ncol;
+    k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk);
+    nf_status rc = nf_scan_u32(ctx, ctx->d_col_nblk, (uint32_t)ncol, ctx->d_col_base, st);
+    if (rc != NF_OK) return rc;
+    k_fill_blocks<<<(ncol + 127) / 128, 128, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk, ctx->d_col_base, ctx->d_blk, ctx->R);
+    const uint32_t bound = (uint32_t)ctx->capBlk;
+    if (ctx->opt_heavy_first) {
+        uint32_t *hist = ctx->d_ctrl + 16;   // 64 words
+        NF_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, 64 * sizeof(uint32_t), st));
+        k_order_hist<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk, hist);
+        k_order_scan<<<1, 32, 0, st>>>(hist);
+        k_order_fill<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk, hist, ctx->d_blk_order);
+    } else {
+        k_order_identity<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk_order);
+    }
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
+
+// ------------------------------------------------------------------------------ A5 + A6
+#define NF_F_NEWBLOCK 1
+#define NF_F_LAST 2
+#define NF_F_EXIT 4
+
+struct __align__(16) StageHdr {
+    int flags;
+    int a, b;          // column image: source column = (cx + a, cy + b) wrapped
+    int zu0, nc;       // unwrapped z index of the first table cell; number of cells in the table
+    uint32_t g_lo;     // first padded slot held by this stage (multiple of 4)
+    int g_cnt;         // slots held
+    uint32_t col, s0, cnt;   // NEWBLOCK: the sink block
+    int pad0, pad1;
+};
+
+struct __align__(128) Stage {
+    float xs[NF_TILE];
+    float ys[NF_TILE];
+    float zs[NF_TILE];
+    uint32_t tab[NF_TABMAX + 1];
+    StageHdr hdr;
+};
+
+struct InteractArgs {
+    const float *sx, *sy, *sz;
+    const uint32_t *skey, *poff, *perm_pad, *order;
+    const NfBlockDesc *blk;
+    uint32_t *ctrl;
+    float *acc;
+    float kfac;
+    NfParams prm;
+};
+
+template <bool NEAR>
+__device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ zs, int lo, int hi,
+                                          float xim, float yi, float zi, float2 &ax, float2 &ay, float2 &az, const float2 c0, const float2 c1,
+                                          const float2 c2) {
+    const float2 nx = make_float2(-xim, -xim), ny = make_float2(-yi, -yi), nz = make_float2(-zi, -zi);
+    const float2 tau = make_float2(NF_TAU, NF_TAU);
+#pragma unroll 4
+    for (int s = lo; s < hi; s += 2) {
+        const float2 X = *reinterpret_cast<const float2 *>(xs + s);
+        const float2 Y = *reinterpret_cast<const float2 *>(ys + s);
+        const float2 Z = *reinterpret_cast<const float2 *>(zs + s);
+        const float2 dx = __fadd2_rn(X, nx), dy = __fadd2_rn(Y, ny), dz = __fadd2_rn(Z, nz);
+        float2 r2 = __ffma2_rn(dx, dx, tau);
+        r2 = __ffma2_rn(dy, dy, r2);
+        r2 = __ffma2_rn(dz, dz, r2);
+        const float2 ri = make_float2(mufu_rsq(r2.x), mufu_rsq(r2.y));
+        const float2 ri2 = __fmul2_rn(ri, ri);
+        float2 f = __fmul2_rn(ri2, ri);                    // r^-3
+        if (NEAR) {
+            const float2 r = __fmul2_rn(r2, ri);           // r
+            float2 h = __ffma2_rn(r, c2, c1);
+            h = __ffma2_rn(r, h, c0);                      // (10 - 15u + 6u^2)/eps^3
+            f.x = fminf(f.x, h.x);                         // Eq. 3 as a min
+            f.y = fminf(f.y, h.y);
+        }
+        ax = __ffma2_rn(f, dx, ax);
+        ay = __ffma2_rn(f, dy, ay);
+        az = __ffma2_rn(f, dz, az);
+    }
+}
+
+__device__ __forceinline__ void fold(float &tot, float &comp, float v, int kahan) {
+    if (kahan) {
+        float y = v - comp;
+        float t = tot + y;
+        comp = (t - tot) - y;
+        tot = t;
+    } else {
+        tot += v;
+    }
+}
+
+__global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArgs A) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    Stage *stages = reinterpret_cast<Stage *>(smem_raw);
+    __shared__ uint64_t full_bar[NF_NSTAGE], empty_bar[NF_NSTAGE];
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int cpd = A.prm.cpd, R = A.prm.R;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NF_NSTAGE; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], NF_NW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    int stage = 0;
+    uint32_t phase = 0;
+
+    if (warp == NF_NW) {
+        // =========================== producer warp ===========================================
+        const uint32_t nblocks = A.ctrl[1];
+        auto emit = [&](int flags, int a, int b, int zu0, int nc, uint32_t tabval, uint32_t g_lo, int g_cnt, uint32_t col, uint32_t s0, uint32_t cnt) {
+            Stage &S = stages[stage];
+            mbar_wait(&empty_bar[stage], phase ^ 1u);
+            S.tab[lane] = tabval;
+            if (lane == 0) {
+                StageHdr h;
+                h.flags = flags; h.a = a; h.b = b; h.zu0 = zu0; h.nc = nc; h.g_lo = g_lo; h.g_cnt = g_cnt;
+                h.col = col; h.s0 = s0; h.cnt = cnt; h.pad0 = 0; h.pad1 = 0;
+                S.hdr = h;
+            }
+            __syncwarp();
+            if (lane == 0) {
+                if (g_cnt > 0) {
+                    const uint32_t bytes = (uint32_t)g_cnt * 4u;
+                    mbar_arrive_expect_tx(&full_bar[stage], 3u * bytes);
+                    bulk_g2s(S.xs, A.sx + g_lo, bytes, &full_bar[stage]);
+                    bulk_g2s(S.ys, A.sy + g_lo, bytes, &full_bar[stage]);
+                    bulk_g2s(S.zs, A.sz + g_lo, bytes, &full_bar[stage]);
+                } else {
+                    mbar_arrive(&full_bar[stage]);
+                }
+            }
+            if (++stage == NF_NSTAGE) { stage = 0; phase ^= 1u; }
+        };
+
+        for (;;) {
+            uint32_t w = 0;
+            if (lane == 0) w = atomicAdd(&A.ctrl[0], 1u);
+            w = __shfl_sync(0xffffffffu, w, 0);
+            if (w >= nblocks) break;
+            const NfBlockDesc d = A.blk[A.order[w]];
+            if (d.cnt == 0) continue;
+            const int ci = (int)(d.col / (uint32_t)cpd), cj = (int)(d.col % (uint32_t)cpd);
+            const int colbase = (int)d.col * cpd;
+            const int Z1 = (int)(A.skey[d.s0] & ~NF_PAD_FLAG) - colbase;
+            const int Z2 = (int)(A.skey[d.s0 + d.cnt - 1] & ~NF_PAD_FLAG) - colbase;
+            int flags = NF_F_NEWBLOCK;
+            for (int a = -R; a <= R; ++a) {
+                int ia; const int sci = nf_wrap1(ci + a, cpd, ia);
+                for (int b = -R; b <= R; ++b) {
+                    int ib; const int scj = nf_wrap1(cj + b, cpd, ib);
+                    const int cb = (sci * cpd + scj) * cpd;
+                    int u = Z1 - R;
+                    const int U1 = Z2 + R;
+                    while (u <= U1) {
+                        const int wz = nf_mod(u, cpd);
+                        int run = U1 - u + 1;
+                        if (run > cpd - wz) run = cpd - wz;
+                        if (run > NF_TABMAX) run = NF_TABMAX;
+                        // table: padded offsets of cells wz .. wz+run (run+1 entries)
+                        const uint32_t tv = A.poff[cb + wz + (lane <= run ? lane : run)];
+                        const uint32_t g0 = __shfl_sync(0xffffffffu, tv, 0);
+                        const uint32_t g1 = __shfl_sync(0xffffffffu, tv, run);
+                        if (g1 > g0) {
+                            const uint32_t gl = g0 & ~3u, ge = (g1 + 3u) & ~3u;
+                            for (uint32_t c0 = gl; c0 < ge; c0 += NF_TILE) {
+                                const uint32_t c1 = (c0 + NF_TILE < ge) ? c0 + NF_TILE : ge;
+                                emit(flags, a, b, u, run, tv, c0, (int)(c1 - c0), d.col, d.s0, d.cnt);
+                                flags = 0;
+                            }
+                        }
+                        u += run;
+                    }
+                }
+            }
+            emit(flags | NF_F_LAST, 0, 0, 0, 0, 0u, 0u, 0, d.col, d.s0, d.cnt);
+        }
+        emit(NF_F_EXIT, 0, 0, 0, 0, 0u, 0u, 0, 0u, 0u, 0u);
+        return;
+    }
+
+    // =============================== consumer warps ==========================================
+    const float2 c0 = make_float2(A.prm.c0, A.prm.c0), c1 = make_float2(A.prm.c1, A.prm.c1), c2 = make_float2(A.prm.c2, A.prm.c2);
+    const int near_cheb = A.prm.near_cheb, kahan = A.prm.kahan;
+    float px = -NF_BIG, py = 0.f, pz = 0.f;
+    int zl = 0, z1 = 0, z2 = -1;
+    bool valid = false, warp_active = false;
+    uint32_t slot = 0;
+    float tx = 0.f, ty = 0.f, tz = 0.f, kx = 0.f, ky = 0.f, kz = 0.f;
+
+    for (;;) {
+        Stage &S = stages[stage];
+        mbar_wait(&full_bar[stage], phase);
+        const StageHdr h = S.hdr;
+        if (h.flags & NF_F_EXIT) break;
+        if (h.flags & NF_F_NEWBLOCK) {
+            const uint32_t off = (uint32_t)(warp * 32 + lane);
+            valid = off < h.cnt;
+            slot = h.s0 + (valid ? off : 0u);
+            const int colbase = (int)h.col * cpd;
+            const uint32_t k = A.skey[slot];
+            zl = (int)(k & ~NF_PAD_FLAG) - colbase;
+            px = valid ? A.sx[slot] : -NF_BIG;
+            py = A.sy[slot];
+            pz = A.sz[slot];
+            const unsigned vm = __ballot_sync(0xffffffffu, valid);
+            warp_active = vm != 0u;
+            if (warp_active) {
+                z1 = __shfl_sync(0xffffffffu, zl, 0);
+                z2 = __shfl_sync(0xffffffffu, zl, 31 - __clz(vm));
+                if (!valid) zl = z2;
+            }
+            tx = ty = tz = kx = ky = kz = 0.f;
+        }
+        if (warp_active && h.g_cnt > 0) {
+            const float xi = px - (float)h.a, yi = py - (float)h.b;
+            const bool near_ab = (abs(h.a) <= near_cheb) && (abs(h.b) <= near_cheb);
+            int zlo = z1 - R, zhi = z2 + R;
+            if (zlo < h.zu0) zlo = h.zu0;
+            if (zhi > h.zu0 + h.nc - 1) zhi = h.zu0 + h.nc - 1;
+            float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax;
+            const uint32_t g_hi = h.g_lo + (uint32_t)h.g_cnt;
+            for (int zu = zlo; zu <= zhi; ++zu) {
+                uint32_t t0 = S.tab[zu - h.zu0], t1 = S.tab[zu - h.zu0 + 1];
+                if (t0 < h.g_lo) t0 = h.g_lo;
+                if (t1 > g_hi) t1 = g_hi;
+                if (t0 >= t1) continue;
+                const int lo = (int)(t0 - h.g_lo), hi = (int)(t1 - h.g_lo);
+                const int dzc = zu - zl;
+                const bool act = valid && (abs(dzc) <= R);
+                const float zi = pz - (float)dzc;
+                const float xim = act ? xi : -NF_BIG;   // masked sink at -BIG, padding sources at +BIG: never coincide
+                const bool near = near_ab && (zu >= z1 - near_cheb) && (zu <= z2 + near_cheb);
+                if (near) pair_loop<true>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2);
+                else pair_loop<false>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2);
+            }
+            fold(tx, kx, ax.x + ax.y, kahan);
+            fold(ty, ky, ay.x + ay.y, kahan);
+            fold(tz, kz, az.x + az.y, kahan);
+        }
+        if (h.flags & NF_F_LAST) {
+            if (valid) {
+                const uint32_t dst = A.perm_pad[slot];
+                if (dst != 0xffffffffu) {
+                    float *o = A.acc + 3ull * dst;
+                    o[0] = A.kfac * tx; o[1] = A.kfac * ty; o[2] = A.kfac * tz;
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_bar[stage]);
+        if (++stage == NF_NSTAGE) { stage = 0; phase ^= 1u; }
+    }
+}
+
+static int g_interact_blocks_per_sm = 0;
+
+nf_status nf_interact_setup(nf_ctx *ctx) {
+    const size_t smem = sizeof(Stage) * NF_NSTAGE;
+    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_interact, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int nb = 0;
+    NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_interact, (NF_NW + 1) * 32, smem));
+    if (nb < 1) { snprintf(ctx->err, sizeof(ctx->err), "interaction kernel does not fit on an SM"); return NF_ECUDA; }
+    g_interact_blocks_per_sm = nb;
+    return NF_OK;
+}
+
+nf_status nf_run_interact(nf_ctx *ctx, int64_t N, float *d_acc, float kfac, cudaStream_t st) {
+    InteractArgs A;
+    A.sx = ctx->d_sorted; A.sy = ctx->d_sorted + ctx->capPad; A.sz = ctx->d_sorted + 2ull * ctx->capPad;
+    A.skey = (const uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
+    A.poff = ctx->d_poff; A.perm_pad = ctx->d_perm_pad; A.order = ctx->d_blk_order; A.blk = ctx->d_blk;
+    A.ctrl = ctx->d_ctrl; A.acc = d_acc; A.kfac = kfac; A.prm = ctx->prm;
+    A.prm.kahan = ctx->opt_kahan;
+    const int grid = ctx->sm_count * g_interact_blocks_per_sm;
+    k_interact<<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A);
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
+
+// ------------------------------------------------------------------------------ exports
+// Neighbour list of one sink cell, enumerated exactly as the producer warp does: column images
+// by nf_wrap1, z by nf_mod of the unwrapped index.
+__global__ void k_neighbors(int cpd, int R, int cell, int32_t *out) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int ck = cell % cpd, cj = (cell / cpd) % cpd, ci = cell / (cpd * cpd);
+    int n = 0;
+    const int w = 2 * R + 1, nn = w * w * w;
+    for (int a = -R; a <= R; ++a) {
+        int ia; const int sci = nf_wrap1(ci + a, cpd, ia);
+        for (int b = -R; b <= R; ++b) {
+            int ib; const int scj = nf_wrap1(cj + b, cpd, ib);
+            const int cb = (sci * cpd + scj) * cpd;
+            for (int u = ck - R; u <= ck + R; ++u, ++n) {
+                const int wz = nf_mod(u, cpd);
+                out[n] = cb + wz;
+                out[nn + 3 * n + 0] = ia;
+                out[nn + 3 * n + 1] = ib;
+                out[nn + 3 * n + 2] = (u - wz) / cpd;
+            }
+        }
+    }
+}
+
+nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st) {
+    k_neighbors<<<1, 32, 0, st>>>(ctx->cpd, ctx->R, cell, ctx->d_nbr);
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
+
+// pairs = sum_c n_c * sum_{c' in N(c)} n_c'   (the caller subtracts N)
+__global__ void __launch_bounds__(256) k_paircount(int cpd, int R, const uint32_t *__restrict__ offsets, unsigned long long *__restrict__ out) {
+    const int ncell = cpd * cpd * cpd;
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long v = 0;
+    if (c < ncell) {
+        const unsigned long long nc = offsets[c + 1] - offsets[c];
+        if (nc) {
+            const int ck = c % cpd, cj = (c / cpd) % cpd, ci = c / (cpd * cpd);
+            unsigned long long s = 0;
+            for (int a = -R; a <= R; ++a) {
+                int ia; const int sci = nf_wrap1(ci + a, cpd, ia);
+                for (int b = -R; b <= R; ++b) {
+                    int ib; const int scj = nf_wrap1(cj + b, cpd, ib);
+                    const int cb = (sci * cpd + scj) * cpd;
+                    for (int u = ck - R; u <= ck + R; ++u) {
+                        const int wz = nf_mod(u, cpd);
+                        s += offsets[cb + wz + 1] - offsets[cb + wz];
+                    }
+                }
+            }
+            v = nc * s;
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(out, v);
+}
+
+nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st) {
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_pairs, 0, sizeof(unsigned long long), st));
+    const int ncell = (int)ctx->ncell;
+    k_paircount<<<(ncell + 255) / 256, 256, 0, st>>>(ctx->cpd, ctx->R, ctx->d_offsets, ctx->d_pairs);
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
