@@ -109,6 +109,10 @@ const char *nf_last_error(const nf_ctx *ctx);
  *   "stage_timing" (0/1)  record CUDA events between stages for nf_stage_ms
  *   "kahan"        (0/1)  compensated fold of per-segment partial sums (default 1)
  *   "heavy_first"  (0/1)  order sink blocks by descending estimated cost (default 1)
+ *   "rc_cells"     (<= 0.25) close-pair radius in cell units: pairs with r < rc are evaluated
+ *                        exactly in double precision instead of the float32 fast path;
+ *                        0 = none (Eq. 3 as a min everywhere); negative (default) = automatic,
+ *                        from the particle-weighted occupancy and eps_s
  * NF_EINVAL: unknown name or value out of range.
  */
 nf_status nf_set_option(nf_ctx *ctx, const char *name, double value);
@@ -136,6 +140,14 @@ nf_status nf_stage_ms(nf_ctx *ctx, float *h_ms /* NF_N_STAGES */);
  */
 nf_status nf_debug_cells(nf_ctx *ctx, const uint32_t **d_offsets, const uint32_t **d_perm,
                          const float **d_sorted, const uint32_t **d_poffsets, int64_t *h_npad);
+
+/* nf_close_radius -- the close-pair radius (cell units) the last nf_accel used; 0 = none
+ * (see option "rc_cells").  Synchronises. */
+nf_status nf_close_radius(nf_ctx *ctx, double *h_rc_cells);
+
+/* nf_launch_count -- number of CUDA kernels this context has launched since nf_create
+ * (memsets and copies are not counted).  bench.py reports the difference over its timed region. */
+nf_status nf_launch_count(nf_ctx *ctx, int64_t *h_count);
 
 /* nf_debug_read -- copy `bytes` from a device pointer handed out by nf_debug_cells to host
  * memory (synchronous).  NF_EINVAL on NULL arguments. */

@@ -21,7 +21,7 @@ STAGE_NAMES = ["A1_key_hist", "A2_scan", "A3_scatter_rank_gather", "A4_scheduler
 # every symbol include/nearfield.h declares
 SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", "nf_sync",
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
-           "nf_interaction_count", "nf_probe_pipes", "nf_debug_read"]
+           "nf_interaction_count", "nf_probe_pipes", "nf_debug_read", "nf_launch_count", "nf_close_radius"]
 
 
 class NearFieldError(RuntimeError):
@@ -66,6 +66,10 @@ def load_library() -> ctypes.CDLL:
     L.nf_debug_neighbors.argtypes = [vp, i32, vp, vp]
     L.nf_interaction_count.restype = i32
     L.nf_interaction_count.argtypes = [vp, ctypes.POINTER(i64)]
+    L.nf_close_radius.restype = i32
+    L.nf_close_radius.argtypes = [vp, ctypes.POINTER(dbl)]
+    L.nf_launch_count.restype = i32
+    L.nf_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     L.nf_debug_read.restype = i32
     L.nf_debug_read.argtypes = [vp, vp, vp, ctypes.c_uint64]
     L.nf_probe_pipes.restype = i32
@@ -168,6 +172,16 @@ class NearField:
         buf = (ctypes.c_float * NF_N_STAGES)()
         self._check(_L.nf_stage_ms(self._h, buf))
         return {STAGE_NAMES[i]: float(buf[i]) for i in range(6)}
+
+    def close_radius(self) -> float:
+        v = ctypes.c_double()
+        self._check(_L.nf_close_radius(self._h, ctypes.byref(v)))
+        return float(v.value)
+
+    def launch_count(self) -> int:
+        v = ctypes.c_int64()
+        self._check(_L.nf_launch_count(self._h, ctypes.byref(v)))
+        return int(v.value)
 
     def interaction_count(self) -> int:
         v = ctypes.c_int64()

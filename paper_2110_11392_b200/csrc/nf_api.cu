@@ -41,11 +41,12 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     c->device = dev; c->cpd = cpd; c->R = R; c->eps_p = eps_plummer; c->box = box; c->gm = 0.0;
     c->sm_count = prop.multiProcessorCount;
     c->ncell = (int64_t)cpd * cpd * cpd; c->ncol = (int64_t)cpd * cpd;
-    c->opt_kahan = 1; c->opt_heavy_first = 1; c->opt_stage_timing = 0;
+    c->opt_kahan = 1; c->opt_heavy_first = 1; c->opt_stage_timing = 0; c->opt_rc = -1.f;
     NfParams &p = c->prm;
     p.cpd = cpd; p.R = R; p.ncell = (int)c->ncell; p.ncol = (int)c->ncol;
     p.scale = (double)cpd / box;
     const double e = NF_SPLINE_PER_PLUMMER * eps_plummer * p.scale;   // eps_s in cell units
+    p.eps_cells = e;
     p.c0 = (float)(10.0 / (e * e * e));
     p.c1 = (float)(-15.0 / (e * e * e * e));
     p.c2 = (float)(6.0 / (e * e * e * e * e));
@@ -106,6 +107,11 @@ extern "C" nf_status nf_set_gm(nf_ctx *c, double gm) {
 extern "C" nf_status nf_set_option(nf_ctx *c, const char *name, double v) {
     if (!c || !name) return NF_EINVAL;
     const int iv = (int)v;
+    if (!strcmp(name, "rc_cells")) {
+        if (!(v <= 0.25) || !isfinite(v)) { snprintf(c->err, sizeof c->err, "nf_set_option(rc_cells): need value <= 0.25 (negative = automatic)"); return NF_EINVAL; }
+        c->opt_rc = (float)v;
+        return NF_OK;
+    }
     if (v != 0.0 && v != 1.0) { snprintf(c->err, sizeof c->err, "nf_set_option(%s): value must be 0 or 1", name); return NF_EINVAL; }
     if (!strcmp(name, "stage_timing")) c->opt_stage_timing = iv;
     else if (!strcmp(name, "kahan")) c->opt_kahan = iv;
@@ -162,7 +168,7 @@ extern "C" nf_status nf_accel(nf_ctx *c, const float *d_pos, int64_t N, float *d
     const double gm = c->gm > 0 ? c->gm : 1.0 / (double)N;
     const double cellsz = c->box / (double)c->cpd;
     const float kfac = (float)(gm / (cellsz * cellsz));
-    rc = nf_run_interact(c, N, d_acc, kfac, st);
+    rc = nf_run_interact(c, d_pos, N, d_acc, kfac, st);
     if (rc != NF_OK) return rc;
     if (c->opt_stage_timing) { cudaEventRecord(c->ev[5], st); cudaEventRecord(c->ev[7], st); }
     return NF_OK;
@@ -222,6 +228,22 @@ extern "C" nf_status nf_debug_cells(nf_ctx *c, const uint32_t **d_offsets, const
     if (d_sorted) *d_sorted = c->d_sorted;
     if (d_poffsets) *d_poffsets = c->d_poff;
     if (h_npad) *h_npad = c->capPad;   // plane stride of d_sorted
+    return NF_OK;
+}
+
+extern "C" nf_status nf_close_radius(nf_ctx *c, double *h_rc_cells) {
+    if (!c || !h_rc_cells) return NF_EINVAL;
+    if (!c->have_last) { snprintf(c->err, sizeof c->err, "nf_close_radius: no nf_accel call yet"); return NF_EINVAL; }
+    NF_CUDA_OK(c, cudaStreamSynchronize(c->last_stream));
+    float dyn[2];
+    NF_CUDA_OK(c, cudaMemcpy(dyn, c->d_ctrl + 96, sizeof dyn, cudaMemcpyDeviceToHost));
+    *h_rc_cells = dyn[1];
+    return NF_OK;
+}
+
+extern "C" nf_status nf_launch_count(nf_ctx *c, int64_t *h_count) {
+    if (!c || !h_count) return NF_EINVAL;
+    *h_count = c->launches;
     return NF_OK;
 }
 

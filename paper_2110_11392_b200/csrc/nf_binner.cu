@@ -149,9 +149,9 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const uint32_t *__r
 static nf_status scan_cells(nf_ctx *ctx, cudaStream_t st) {
     uint32_t n = (uint32_t)ctx->ncell;
     uint32_t nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
-    k_scan_reduce<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk);
-    k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(ctx->d_scan_blk, nblk);
-    k_scan_apply<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk, ctx->d_offsets, ctx->d_poff, ctx->d_ctrl);
+    k_scan_reduce<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk); ctx->launches++;
+    k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(ctx->d_scan_blk, nblk); ctx->launches++;
+    k_scan_apply<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk, ctx->d_offsets, ctx->d_poff, ctx->d_ctrl); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }
@@ -159,9 +159,9 @@ static nf_status scan_cells(nf_ctx *ctx, cudaStream_t st) {
 nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st) {
     // exclusive scan of n uint32 values into out[0..n]; the total also goes to ctrl[1]
     uint32_t nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
-    k_scan_reduce<1><<<nblk, SCAN_THREADS, 0, st>>>(in, n, ctx->d_scan_blk);
-    k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(ctx->d_scan_blk, nblk);
-    k_scan_apply<1><<<nblk, SCAN_THREADS, 0, st>>>(in, n, ctx->d_scan_blk, out, nullptr, ctx->d_ctrl);
+    k_scan_reduce<1><<<nblk, SCAN_THREADS, 0, st>>>(in, n, ctx->d_scan_blk); ctx->launches++;
+    k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(ctx->d_scan_blk, nblk); ctx->launches++;
+    k_scan_apply<1><<<nblk, SCAN_THREADS, 0, st>>>(in, n, ctx->d_scan_blk, out, nullptr, ctx->d_ctrl); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }
@@ -225,21 +225,21 @@ nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t
     NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_counts, 0, (size_t)(ctx->ncell + 1) * sizeof(uint32_t), st));
     NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_ctrl, 0, 16 * sizeof(uint32_t), st));
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[0], st);
-    k_key_hist<<<(n + 255) / 256, 256, 0, st>>>(d_pos, n, ctx->prm.scale, ctx->cpd, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_ctrl);
+    k_key_hist<<<(n + 255) / 256, 256, 0, st>>>(d_pos, n, ctx->prm.scale, ctx->cpd, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_ctrl); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[1], st);
     nf_status rc = scan_cells(ctx, st);
     if (rc != NF_OK) return rc;
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[2], st);
     uint32_t *skey = (uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
-    k_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_poff, ctx->d_tmp_perm, skey);
+    k_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_poff, ctx->d_tmp_perm, skey); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     // upper bound of the padded slot count: N + ncell (+8 slack), known on the host
     uint64_t bound = (uint64_t)N + (uint64_t)ctx->ncell + 8;
     if (bound > (uint64_t)ctx->capPad) bound = ctx->capPad;
     k_rank_gather<<<(uint32_t)((bound + 255) / 256), 256, 0, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl,
                                                                    ctx->d_offsets, ctx->d_poff, ctx->d_tmp_perm, ctx->d_sorted,
-                                                                   ctx->d_perm_true, ctx->d_perm_pad);
+                                                                   ctx->d_perm_true, ctx->d_perm_pad); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[3], st);
     return NF_OK;

@@ -26,6 +26,7 @@
 struct NfParams {
     int cpd, R, ncell, ncol;
     double scale;        // cpd / box
+    double eps_cells;    // eps_s in cell units
     float c0, c1, c2;    // spline coefficients in cell units: 10/e^3, -15/e^4, 6/e^5, e = eps_s/cell
     int near_cheb;       // source cells at Chebyshev distance <= near_cheb may hold r < eps_s
     int kahan;
@@ -45,6 +46,7 @@ struct nf_ctx {
     NfParams prm;
     // options
     int opt_stage_timing, opt_kahan, opt_heavy_first;
+    float opt_rc;                // close-pair radius in cells; < 0 = automatic
     // scratch (grow-only)
     int64_t capN, capPad, capBlk;
     uint32_t *d_key, *d_arr, *d_counts, *d_offsets, *d_poff, *d_tmp_perm, *d_perm_true, *d_perm_pad;
@@ -53,6 +55,7 @@ struct nf_ctx {
     uint32_t *d_col_nblk, *d_col_base, *d_scan32_blk, *d_blk_order;
     NfBlockDesc *d_blk;
     uint32_t *d_ctrl;            // [0] work counter  [1] number of blocks  [2] bad-position flag  [3] npad
+                                 // [16..79] cost histogram  [96..97] float rc^2, rc  [100..101] u64 sum n_c^2
     unsigned long long *d_pairs;
     int32_t *d_nbr;              // debug neighbour list
     // host staging for nf_accel_host
@@ -63,6 +66,7 @@ struct nf_ctx {
     cudaStream_t last_stream;
     int64_t lastN;
     int have_last;
+    int64_t launches;            // kernels launched by this context (nf_launch_count)
     cudaEvent_t ev[8];
     char err[512];
 };
@@ -80,7 +84,7 @@ struct nf_ctx {
 // stages implemented in the other translation units
 nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st);
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st);
-nf_status nf_run_interact(nf_ctx *ctx, int64_t N, float *d_acc, float kfac, cudaStream_t st);
+nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc, float kfac, cudaStream_t st);
 nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st);
 nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_interact_setup(nf_ctx *ctx);

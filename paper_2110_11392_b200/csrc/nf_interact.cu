@@ -113,23 +113,62 @@ __global__ void __launch_bounds__(256) k_order_identity(const uint32_t *__restri
     if (b < ctrl[1]) order[b] = b;
 }
 
-nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st);
+// Close-pair radius r_c.  Per-pair error model of the float32 fast path:
+// relative error kappa(r) = 1e-6 (MUFU.RSQ cubed + roundings) + 1.2e-7/r (float32 offsets of both
+// particles, up to 1.5e-8 cell each, and the shifted sink, up to 3e-8, against a separation r).
+// A pair with F = 1/r^2 is sent to close_pair() when F kappa(r) > 0.4e-5 rms|a|, with the
+// Holtsmark-like estimate rms|a|^2 ~ 4 pi n_pw / eps_s (cell units; n_pw = sum n_c^2 / N, the
+// particle-weighted cell occupancy; measured rms is ~1.4x this, so the estimate is conservative).
+// If even the softened core needs no exact path, r_c = 0 and Eq. 3 is evaluated as a min.
+__global__ void __launch_bounds__(256) k_density(int ncell, const uint32_t *__restrict__ counts, unsigned long long *__restrict__ sum2) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long v = 0;
+    if (c < ncell) { unsigned long long n = counts[c]; v = n * n; }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(sum2, v);
+}
+__global__ void k_choose_rc(const unsigned long long *__restrict__ sum2, double N, double eps_cells, float rc_override, float *__restrict__ dyn) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double rc;
+    if (rc_override >= 0.f) {
+        rc = rc_override;
+    } else {
+        const double npw = (double)(*sum2) / N;
+        const double rms = sqrt(4.0 * 3.14159265358979 * npw / eps_cells);
+        const double budget = 0.4e-5 * rms;
+        rc = 0.05;
+        for (int it = 0; it < 20; ++it) rc = sqrt((1.0e-6 + 1.2e-7 / rc) / budget);
+        if (rc < eps_cells) {
+            // inside the core F <= 2.01/eps^2 and |dF/dr| <= 10/eps^3
+            const double core = 2.01 / (eps_cells * eps_cells) * 1.0e-6 + 10.0 / (eps_cells * eps_cells * eps_cells) * 6.0e-8;
+            rc = (core <= budget) ? 0.0 : eps_cells;
+        }
+        if (rc > 0.25) rc = 0.25;
+    }
+    dyn[0] = (float)(rc * rc);
+    dyn[1] = (float)rc;
+}
 
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st) {
     const int ncol = (int)ctx->ncol;
-    k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk);
+    unsigned long long *sum2 = (unsigned long long *)(ctx->d_ctrl + 100);
+    NF_CUDA_OK(ctx, cudaMemsetAsync(sum2, 0, 8, st));
+    k_density<<<((int)ctx->ncell + 255) / 256, 256, 0, st>>>((int)ctx->ncell, ctx->d_counts, sum2); ctx->launches++;
+    k_choose_rc<<<1, 32, 0, st>>>(sum2, (double)N, ctx->prm.eps_cells, ctx->opt_rc, (float *)(ctx->d_ctrl + 96)); ctx->launches++;
+    k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk); ctx->launches++;
     nf_status rc = nf_scan_u32(ctx, ctx->d_col_nblk, (uint32_t)ncol, ctx->d_col_base, st);
     if (rc != NF_OK) return rc;
-    k_fill_blocks<<<(ncol + 127) / 128, 128, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk, ctx->d_col_base, ctx->d_blk, ctx->R);
+    k_fill_blocks<<<(ncol + 127) / 128, 128, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk, ctx->d_col_base, ctx->d_blk, ctx->R); ctx->launches++;
     const uint32_t bound = (uint32_t)ctx->capBlk;
     if (ctx->opt_heavy_first) {
         uint32_t *hist = ctx->d_ctrl + 16;   // 64 words
         NF_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, 64 * sizeof(uint32_t), st));
-        k_order_hist<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk, hist);
-        k_order_scan<<<1, 32, 0, st>>>(hist);
-        k_order_fill<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk, hist, ctx->d_blk_order);
+        k_order_hist<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk, hist); ctx->launches++;
+        k_order_scan<<<1, 32, 0, st>>>(hist); ctx->launches++;
+        k_order_fill<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk, hist, ctx->d_blk_order); ctx->launches++;
     } else {
-        k_order_identity<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk_order);
+        k_order_identity<<<(bound + 255) / 256, 256, 0, st>>>(ctx->d_ctrl, ctx->d_blk_order); ctx->launches++;
     }
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
@@ -159,19 +198,74 @@ struct __align__(128) Stage {
 };
 
 struct InteractArgs {
-    const float *sx, *sy, *sz;
+    const float *sx, *sy, *sz, *pos;
     const uint32_t *skey, *poff, *perm_pad, *order;
     const NfBlockDesc *blk;
     uint32_t *ctrl;
+    const float *dyn;        // [0] rc^2 (cell units^2; 0 = no close-pair radius, use the min form)
     float *acc;
     float kfac;
     NfParams prm;
 };
 
-template <bool NEAR>
+// Exact evaluation of one close pair (r < r_c) in double precision.  The float32 cell-relative
+// offsets of the sorted planes are NOT enough here: for x < box/4 the input float32 position is
+// finer than a float32 offset of magnitude ~0.5 cell, and 1.5e-8 cell is 3e-6 of the force of a
+// pair 0.01 cell apart.  So both particles are re-read from the caller's position array through
+// the permutation and their offsets recomputed in double; the INTEGER cell shift is added last.
+// Piecewise Eq. 3.  Rare (a few per cent of the sinks have such a neighbour),
+// hence noinline and out of the hot loop.
+struct CloseCtx {
+    const float *pos;          // caller's positions (input order)
+    const uint32_t *perm_pad;  // padded slot -> input index
+    double scale;              // cpd / box
+    double eps;                // eps_s in cell units
+    uint32_t sink_slot;
+    int have_p;                // exact sink offsets cached?
+    double opx, opy, opz;      // exact sink offsets (cell units)
+    int a, b, dzc;             // integer cell shift of the source cell relative to the sink's cell
+    double sx, sy, sz;         // accumulated exact contributions
+};
+__device__ __forceinline__ double exact_offset(float x, double scale) {
+    const double t = (double)x * scale;
+    return t - floor(t) - 0.5;
+}
+__device__ __noinline__ void close_pair(CloseCtx &C, uint32_t src_slot) {
+    // padding slots (input index 0xffffffff) sit at +BIG: a padding SINK meets padding sources at d = 0
+    const uint32_t qi = C.perm_pad[src_slot];
+    if (qi == 0xffffffffu) return;
+    if (!C.have_p) {
+        const uint32_t pi = C.perm_pad[C.sink_slot];
+        if (pi == 0xffffffffu) return;
+        const float *p = C.pos + 3ull * pi;
+        C.opx = exact_offset(p[0], C.scale); C.opy = exact_offset(p[1], C.scale); C.opz = exact_offset(p[2], C.scale);
+        C.have_p = 1;
+    }
+    const float *q = C.pos + 3ull * qi;
+    const double dx = (exact_offset(q[0], C.scale) - C.opx) + (double)C.a;
+    const double dy = (exact_offset(q[1], C.scale) - C.opy) + (double)C.b;
+    const double dz = (exact_offset(q[2], C.scale) - C.opz) + (double)C.dzc;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    if (r2 == 0.0) return;                       // self pair / coincident particles: F(0) = 0
+    const double r = sqrt(r2);
+    double f;
+    if (r < C.eps) {
+        const double u = r / C.eps;
+        f = (10.0 - 15.0 * u + 6.0 * u * u) / (C.eps * C.eps * C.eps);
+    } else {
+        f = 1.0 / (r2 * r);
+    }
+    C.sx += f * dx; C.sy += f * dy; C.sz += f * dz;
+}
+
+// MODE 0: far cells, pure r^-3 (11 FMA-pipe ops per pair)
+// MODE 1: near cells, Eq. 3 as min(r^-3, spline) (14 ops)            -- used when no close-pair radius is needed
+// MODE 2: near cells, r^-3 with pairs r^2 < rc2 zeroed and sent to close_pair()
+// MODE 3: as 2 for source cells that contain the sinks themselves (r^2 == 0 is not sent)
+template <int MODE>
 __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ zs, int lo, int hi,
                                           float xim, float yi, float zi, float2 &ax, float2 &ay, float2 &az, const float2 c0, const float2 c1,
-                                          const float2 c2) {
+                                          const float2 c2, const float rc2, CloseCtx &C, const uint32_t g_lo) {
     const float2 nx = make_float2(-xim, -xim), ny = make_float2(-yi, -yi), nz = make_float2(-zi, -zi);
     const float2 tau = make_float2(NF_TAU, NF_TAU);
 #pragma unroll 4
@@ -186,12 +280,21 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
         const float2 ri = make_float2(mufu_rsq(r2.x), mufu_rsq(r2.y));
         const float2 ri2 = __fmul2_rn(ri, ri);
         float2 f = __fmul2_rn(ri2, ri);                    // r^-3
-        if (NEAR) {
+        if (MODE == 1) {
             const float2 r = __fmul2_rn(r2, ri);           // r
             float2 h = __ffma2_rn(r, c2, c1);
             h = __ffma2_rn(r, h, c0);                      // (10 - 15u + 6u^2)/eps^3
             f.x = fminf(f.x, h.x);                         // Eq. 3 as a min
             f.y = fminf(f.y, h.y);
+        }
+        if (MODE >= 2) {
+            const bool p0 = r2.x < rc2, p1 = r2.y < rc2;
+            f.x = p0 ? 0.f : f.x;
+            f.y = p1 ? 0.f : f.y;
+            if (p0 | p1) {
+                if (p0 && (MODE == 2 || r2.x > 2.f * NF_TAU)) close_pair(C, g_lo + (uint32_t)s);
+                if (p1 && (MODE == 2 || r2.y > 2.f * NF_TAU)) close_pair(C, g_lo + (uint32_t)s + 1u);
+            }
         }
         ax = __ffma2_rn(f, dx, ax);
         ay = __ffma2_rn(f, dy, ay);
@@ -308,6 +411,11 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
     // =============================== consumer warps ==========================================
     const float2 c0 = make_float2(A.prm.c0, A.prm.c0), c1 = make_float2(A.prm.c1, A.prm.c1), c2 = make_float2(A.prm.c2, A.prm.c2);
     const int near_cheb = A.prm.near_cheb, kahan = A.prm.kahan;
+    const float rc2 = A.dyn[0];
+    const bool flagmode = rc2 > 0.f;
+    CloseCtx C;
+    C.pos = A.pos; C.perm_pad = A.perm_pad; C.scale = A.prm.scale; C.eps = A.prm.eps_cells;
+    C.sx = C.sy = C.sz = 0.0; C.opx = C.opy = C.opz = 0.0; C.have_p = 0; C.sink_slot = 0; C.a = C.b = C.dzc = 0;
     float px = -NF_BIG, py = 0.f, pz = 0.f;
     int zl = 0, z1 = 0, z2 = -1;
     bool valid = false, warp_active = false;
@@ -337,9 +445,11 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
                 if (!valid) zl = z2;
             }
             tx = ty = tz = kx = ky = kz = 0.f;
+            C.sink_slot = slot; C.have_p = 0; C.sx = C.sy = C.sz = 0.0;
         }
         if (warp_active && h.g_cnt > 0) {
             const float xi = px - (float)h.a, yi = py - (float)h.b;
+            C.a = h.a; C.b = h.b;
             const bool near_ab = (abs(h.a) <= near_cheb) && (abs(h.b) <= near_cheb);
             int zlo = z1 - R, zhi = z2 + R;
             if (zlo < h.zu0) zlo = h.zu0;
@@ -357,8 +467,11 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
                 const float zi = pz - (float)dzc;
                 const float xim = act ? xi : -NF_BIG;   // masked sink at -BIG, padding sources at +BIG: never coincide
                 const bool near = near_ab && (zu >= z1 - near_cheb) && (zu <= z2 + near_cheb);
-                if (near) pair_loop<true>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2);
-                else pair_loop<false>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2);
+                C.dzc = dzc;
+                if (!near) pair_loop<0>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, rc2, C, h.g_lo);
+                else if (!flagmode) pair_loop<1>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, rc2, C, h.g_lo);
+                else if (h.a == 0 && h.b == 0 && zu >= z1 && zu <= z2) pair_loop<3>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, rc2, C, h.g_lo);
+                else pair_loop<2>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, rc2, C, h.g_lo);
             }
             fold(tx, kx, ax.x + ax.y, kahan);
             fold(ty, ky, ay.x + ay.y, kahan);
@@ -369,7 +482,9 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
                 const uint32_t dst = A.perm_pad[slot];
                 if (dst != 0xffffffffu) {
                     float *o = A.acc + 3ull * dst;
-                    o[0] = A.kfac * tx; o[1] = A.kfac * ty; o[2] = A.kfac * tz;
+                    o[0] = (float)((double)A.kfac * ((double)tx + C.sx));
+                    o[1] = (float)((double)A.kfac * ((double)ty + C.sy));
+                    o[2] = (float)((double)A.kfac * ((double)tz + C.sz));
                 }
             }
         }
@@ -391,15 +506,16 @@ nf_status nf_interact_setup(nf_ctx *ctx) {
     return NF_OK;
 }
 
-nf_status nf_run_interact(nf_ctx *ctx, int64_t N, float *d_acc, float kfac, cudaStream_t st) {
+nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc, float kfac, cudaStream_t st) {
     InteractArgs A;
+    A.pos = d_pos;
     A.sx = ctx->d_sorted; A.sy = ctx->d_sorted + ctx->capPad; A.sz = ctx->d_sorted + 2ull * ctx->capPad;
     A.skey = (const uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
     A.poff = ctx->d_poff; A.perm_pad = ctx->d_perm_pad; A.order = ctx->d_blk_order; A.blk = ctx->d_blk;
-    A.ctrl = ctx->d_ctrl; A.acc = d_acc; A.kfac = kfac; A.prm = ctx->prm;
+    A.ctrl = ctx->d_ctrl; A.dyn = (const float *)(ctx->d_ctrl + 96); A.acc = d_acc; A.kfac = kfac; A.prm = ctx->prm;
     A.prm.kahan = ctx->opt_kahan;
     const int grid = ctx->sm_count * g_interact_blocks_per_sm;
-    k_interact<<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A);
+    k_interact<<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }
@@ -429,7 +545,7 @@ __global__ void k_neighbors(int cpd, int R, int cell, int32_t *out) {
 }
 
 nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st) {
-    k_neighbors<<<1, 32, 0, st>>>(ctx->cpd, ctx->R, cell, ctx->d_nbr);
+    k_neighbors<<<1, 32, 0, st>>>(ctx->cpd, ctx->R, cell, ctx->d_nbr); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }
@@ -466,7 +582,7 @@ __global__ void __launch_bounds__(256) k_paircount(int cpd, int R, const uint32_
 nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st) {
     NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_pairs, 0, sizeof(unsigned long long), st));
     const int ncell = (int)ctx->ncell;
-    k_paircount<<<(ncell + 255) / 256, 256, 0, st>>>(ctx->cpd, ctx->R, ctx->d_offsets, ctx->d_pairs);
+    k_paircount<<<(ncell + 255) / 256, 256, 0, st>>>(ctx->cpd, ctx->R, ctx->d_offsets, ctx->d_pairs); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }
