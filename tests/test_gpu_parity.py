@@ -1,0 +1,320 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): per-particle |da| <= 1e-5 * rms|a| and median relative error
+<= 2e-6 (definitions: DESIGN.md reading S13); cell offsets, permutation, neighbour lists and
+pair counts bit-exact.  Small cases are compared element by element on every particle; the
+full-size configs on seeded sink-cell samples the oracle can evaluate (all their sources
+included) plus properties that hold at any size.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2110_11392_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_ABS = 1e-5      # x rms|a|
+TOL_MED = 2e-6
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    torch.cuda.set_device(0)
+    return torch
+
+
+@pytest.fixture(scope="module")
+def NF():
+    from paper_2110_11392_b200.binding import NearField
+    return NearField
+
+
+def gpu_accel(torch, NF, pos, cpd, R, eps_p, gm=None, opts=None, want_debug=False):
+    with NF(cpd, R, eps_p, 1.0) as nf:
+        if gm is not None:
+            nf.set_gm(gm)
+        for k, v in (opts or {}).items():
+            nf.set_option(k, v)
+        acc = nf.accel(torch.from_numpy(np.ascontiguousarray(pos, dtype=np.float32)).cuda())
+        nf.sync()
+        out = acc.cpu().numpy().astype(np.float64)
+        pairs = nf.interaction_count() if len(pos) else 0
+        dbg = nf.debug_cells() if want_debug and len(pos) else None
+    return out, pairs, dbg
+
+
+def check(got, ref, sel=None, label=""):
+    if sel is not None:
+        got, ref = got[sel], ref[sel]
+    d = np.linalg.norm(got - ref, axis=1)
+    a = np.linalg.norm(ref, axis=1)
+    rms = np.sqrt((a ** 2).mean())
+    assert np.isfinite(got).all(), label
+    if rms == 0:
+        assert np.all(got == 0), label
+        return 0.0, 0.0
+    worst = d.max() / rms
+    med = np.median(d[a > 0] / a[a > 0])
+    assert worst <= TOL_ABS, f"{label}: max |da| = {worst:.3e} rms|a| (> {TOL_ABS})"
+    assert med <= TOL_MED, f"{label}: median relative error {med:.3e} (> {TOL_MED})"
+    return worst, med
+
+
+# ----------------------------------------------------------------------------- small: every particle
+SMALL = [
+    ("cfg1 full", W.CONFIGS[1]),
+    ("cfg2 @cpd13", W.scaled(W.CONFIGS[2], 13)),
+    ("cfg3 @cpd10", W.scaled(W.CONFIGS[3], 10)),
+    ("cfg4 @cpd9", W.scaled(W.CONFIGS[4], 9)),
+    ("cfg5 @cpd9 R3", W.scaled(W.CONFIGS[5], 9)),
+    ("cfg2 @cpd5 (=2R+1)", W.scaled(W.CONFIGS[2], 5)),
+    ("cfg5 @cpd7 R3 (=2R+1)", W.scaled(W.CONFIGS[5], 7)),
+    ("cfg2 @cpd6 even", W.scaled(W.CONFIGS[2], 6, seed=3)),
+]
+
+
+@pytest.mark.parametrize("label,cfg", SMALL, ids=[s[0] for s in SMALL])
+def test_small_configs_elementwise(torch_cuda, NF, oracle_mod, label, cfg):
+    pos = W.make_positions(cfg)
+    got, pairs, dbg = gpu_accel(torch_cuda, NF, pos, cfg.cpd, cfg.R, cfg.eps_p, want_debug=True)
+    ref, ref_pairs = oracle_mod.accel(pos, cfg.cpd, cfg.R, cfg.eps_p)
+    assert pairs == ref_pairs                                   # integer work count, bit exact
+    cell, off = oracle_mod.bin_particles(pos, cfg.cpd)
+    offsets, order = oracle_mod.cell_lists(cell, cfg.cpd)
+    assert np.array_equal(dbg["offsets"].astype(np.int64), offsets)          # binning bit exact
+    assert np.array_equal(dbg["perm"].astype(np.int64), order)               # stable order bit exact
+    check(got, ref, label=label)
+    # momentum: symmetric neighbour relation (float32 sums => tolerance, not 1e-15)
+    assert np.abs(got.sum(0)).max() <= 2e-6 * np.abs(got).sum()
+
+
+def test_sorted_planes_hold_cell_relative_offsets(torch_cuda, NF, oracle_mod):
+    cfg = W.scaled(W.CONFIGS[2], 8)        # cell = 1/8: offsets exact in float32
+    pos = W.make_positions(cfg)
+    _, _, dbg = gpu_accel(torch_cuda, NF, pos, cfg.cpd, cfg.R, cfg.eps_p, want_debug=True)
+    cell, off = oracle_mod.bin_particles(pos, cfg.cpd)
+    offsets, order = oracle_mod.cell_lists(cell, cfg.cpd)
+    key = dbg["sorted_key"]
+    real = (key & 0x80000000) == 0
+    assert real.sum() == cfg.N and np.all(dbg["poffsets"] % 2 == 0)
+    assert np.array_equal(key[real].astype(np.int64), cell[order])
+    want = (off[order] * cfg.cpd).astype(np.float32)                          # cell units, rounded once
+    assert np.array_equal(dbg["sorted_xyz"][real], want)
+    assert np.all(np.abs(dbg["sorted_xyz"][real]) <= 0.5)
+    assert np.all(dbg["sorted_xyz"][~real][:, 0] > 1e17)                      # padding sits at +BIG
+
+
+@pytest.mark.parametrize("cpd,R", [(7, 2), (9, 3), (5, 2), (3, 1), (12, 4)])
+def test_neighbor_lists_bit_exact(torch_cuda, NF, oracle_mod, cpd, R):
+    with NF(cpd, R, 0.01, 1.0) as nf:
+        for cell in sorted({0, cpd ** 3 - 1, cpd ** 3 // 2, cpd - 1, cpd * cpd - 1, (cpd - 1) * cpd * cpd}):
+            ids, img = nf.debug_neighbors(cell)
+            oids, oimg = oracle_mod.neighbors(cpd, R, cell)
+            assert np.array_equal(ids, oids) and np.array_equal(img, oimg), (cpd, R, cell)
+
+
+# ----------------------------------------------------------------------------- pins re-run on the GPU
+def test_two_particle_closed_form_on_gpu(torch_cuda, NF, oracle_mod):
+    tab = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "eq3_force_table.txt"))
+    cpd, R, eps_p = 8, 2, 0.02
+    eps_s = 2.16 * eps_p
+    for rc in (-1.0, 0.0):                           # exact close-pair path / min form of Eq. 3
+        for u, g in tab:
+            if u * eps_s > 0.12:
+                continue
+            n = np.array([2.0, -1.0, 2.0]) / 3.0
+            x1 = np.array([0.52, 0.58, 0.53])
+            pos = np.array([x1, x1 + u * eps_s * n], dtype=np.float32)
+            got, pairs, _ = gpu_accel(torch_cuda, NF, pos, cpd, R, eps_p, gm=1.0, opts={"rc_cells": rc})
+            assert pairs == 2
+            a1 = np.linalg.norm(got[0]) * eps_s ** 2
+            assert a1 == pytest.approx(g, rel=3e-5)
+            ref, _ = oracle_mod.accel(pos, cpd, R, eps_p, gm=1.0)
+            assert np.allclose(got, ref, rtol=3e-6, atol=0)
+            assert np.allclose(got[0], -got[1], rtol=1e-6)
+
+
+def test_cutoff_wrap_and_lattice_on_gpu(torch_cuda, NF):
+    cpd, R, c = 16, 2, 1.0 / 16
+    got, pairs, _ = gpu_accel(torch_cuda, NF, np.array([[4 * c + 0.999 * c, 0.3, 0.3], [7 * c + 0.001 * c, 0.3, 0.3]]), cpd, R, 1e-3, gm=1.0)
+    assert pairs == 0 and np.all(got == 0)                                  # delta = R+1 cells: no interaction
+    pos = np.array([[0.01, 0.5, 0.5], [0.99, 0.5, 0.5]], dtype=np.float32)
+    got, pairs, _ = gpu_accel(torch_cuda, NF, pos, 7, 2, 1e-4, gm=1.0)
+    r = (float(pos[0, 0]) + 1.0) - float(pos[1, 0])
+    assert pairs == 2 and got[0, 0] == pytest.approx(-1 / r ** 2, rel=2e-6) and got[1, 0] == pytest.approx(1 / r ** 2, rel=2e-6)
+    g = (np.arange(8) + 0.5) / 8                                            # one particle per cell: force free
+    lat = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    got, pairs, _ = gpu_accel(torch_cuda, NF, lat, 8, 2, 0.01, gm=1.0)
+    assert pairs == 512 * 124 and np.abs(got).max() <= 2e-5 * 64
+
+
+# ----------------------------------------------------------------------------- edge cases
+def test_empty_single_and_degenerate_inputs(torch_cuda, NF, oracle_mod):
+    torch = torch_cuda
+    with NF(7, 2, 0.01, 1.0) as nf:
+        out = nf.accel(torch.empty((0, 3), dtype=torch.float32, device="cuda"))
+        assert out.shape == (0, 3)
+        nf.sync()
+    got, pairs, _ = gpu_accel(torch, NF, np.array([[0.3, 0.4, 0.5]]), 7, 2, 0.01)
+    assert pairs == 0 and np.all(got == 0)
+    # everything in one cell (all other cells empty), odd and even counts, coincident particles
+    rng = np.random.default_rng(4)
+    for n in (2, 3, 33, 64, 257):
+        pos = ((3 + rng.random((n, 3))) / 7).astype(np.float32)
+        pos[-1] = pos[0]                                                   # coincident pair contributes 0
+        got, pairs, _ = gpu_accel(torch, NF, pos, 7, 2, 0.002)
+        ref, rp = oracle_mod.accel(pos, 7, 2, 0.002)
+        assert pairs == rp == n * (n - 1)
+        check(got, ref, label=f"one cell n={n}")
+    # finite positions outside [0, box) are wrapped periodically (reading S5)
+    cfg = W.scaled(W.CONFIGS[2], 7)
+    pos = W.make_positions(cfg)
+    shifted = pos.copy()
+    shifted[::3] += np.float32(1.0)
+    shifted[1::3] -= np.float32(2.0)
+    got, _, _ = gpu_accel(torch, NF, shifted, cfg.cpd, cfg.R, cfg.eps_p)
+    ref, _ = oracle_mod.accel(shifted, cfg.cpd, cfg.R, cfg.eps_p)
+    check(got, ref, label="wrapped positions")
+
+
+def test_heavy_cell_chunking_and_ragged_tiles(torch_cuda, NF, oracle_mod):
+    # one cell with 2600 particles (> 2 tiles of 1024 sources), odd counts next to it, empty cells elsewhere
+    rng = np.random.default_rng(8)
+    cpd = 6
+    heavy = ((2 + rng.random((2601, 3))) / cpd).astype(np.float32)
+    side = ((np.array([3, 2, 2]) + rng.random((37, 3))) / cpd).astype(np.float32)
+    far = ((np.array([5, 5, 0]) + rng.random((5, 3))) / cpd).astype(np.float32)
+    pos = np.concatenate([heavy, side, far])
+    got, pairs, _ = gpu_accel(torch_cuda, NF, pos, cpd, 2, 0.001)
+    ref, rp = oracle_mod.accel(pos, cpd, 2, 0.001)
+    assert pairs == rp
+    check(got, ref, label="heavy cell")
+
+
+def test_nonfinite_position_is_reported(torch_cuda, NF):
+    from paper_2110_11392_b200.binding import NearFieldError, NF_EPOS
+    pos = W.uniform(1000, 2)
+    pos[17, 1] = np.nan
+    with NF(7, 2, 0.01, 1.0) as nf:
+        nf.accel(torch_cuda.from_numpy(pos).cuda())
+        with pytest.raises(NearFieldError) as e:
+            nf.sync()
+        assert e.value.status == NF_EPOS
+
+
+def test_bad_arguments_on_gpu(torch_cuda, NF):
+    from paper_2110_11392_b200.binding import NearFieldError, NF_EINVAL
+    with NF(7, 2, 0.01, 1.0) as nf:
+        with pytest.raises(NearFieldError) as e:
+            nf.accel_ptr(0, 10, 0)
+        assert e.value.status == NF_EINVAL
+        with pytest.raises(NearFieldError):
+            nf.accel_ptr(0, -1, 0)
+        with pytest.raises(NearFieldError):
+            nf.set_option("no_such_option", 1)
+        with pytest.raises(ValueError):
+            nf.accel(torch_cuda.zeros((4, 3), dtype=torch_cuda.float64, device="cuda"))
+
+
+def test_determinism_order_invariance_and_reuse(torch_cuda, NF):
+    torch = torch_cuda
+    cfg = W.scaled(W.CONFIGS[3], 8)
+    pos = W.make_positions(cfg)
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        d = torch.from_numpy(pos).cuda()
+        a0 = nf.accel(d).clone()
+        a1 = nf.accel(d).clone()                      # same handle, second call
+        nf.sync()
+        assert torch.equal(a0, a1)                    # run-to-run bit identical (stable sort, fixed order of sums)
+        perm = np.random.default_rng(1).permutation(cfg.N)
+        a2 = nf.accel(torch.from_numpy(pos[perm]).cuda())
+        nf.sync()
+        a0p = a0.cpu().numpy()[perm]
+        a2 = a2.cpu().numpy()
+        rms = np.sqrt((a0p.astype(np.float64) ** 2).sum(1).mean())
+        assert np.abs(a2 - a0p).max() <= 2e-6 * rms   # P10: within-cell order changes the sum order only
+        # smaller N after larger N on the same handle (scratch is grow-only)
+        small = W.uniform(500, 5)
+        a3 = nf.accel(torch.from_numpy(small).cuda()).cpu().numpy()
+    got, _, _ = gpu_accel(torch, NF, small, cfg.cpd, cfg.R, cfg.eps_p)
+    assert np.array_equal(a3.astype(np.float64), got)
+
+
+def test_host_buffer_entry_point_matches_device_one(torch_cuda, NF):
+    cfg = W.scaled(W.CONFIGS[2], 9)
+    pos = W.make_positions(cfg)
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        h = nf.accel_host(pos)
+        d = nf.accel(torch_cuda.from_numpy(pos).cuda()).cpu().numpy()
+    assert np.array_equal(h, d)
+
+
+def test_user_stream_and_stage_times(torch_cuda, NF):
+    torch = torch_cuda
+    cfg = W.scaled(W.CONFIGS[2], 9)
+    pos = torch.from_numpy(W.make_positions(cfg)).cuda()
+    st = torch.cuda.Stream()
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        nf.set_option("stage_timing", 1)
+        n0 = nf.launch_count()
+        with torch.cuda.stream(st):
+            a = nf.accel(pos, stream=st)
+        st.synchronize()
+        ms = nf.stage_ms()
+        assert nf.launch_count() - n0 >= 10
+        assert ms["total"] > 0 and ms["A5_interact_A6_unpermute"] > 0 and ms["total"] >= ms["A5_interact_A6_unpermute"]
+        b = nf.accel(pos)
+        torch.cuda.synchronize()
+        assert torch.equal(a, b)
+
+
+# ----------------------------------------------------------------------------- full-size configs (sampled)
+def _sample_cells(cfg, counts, n_random, n_extreme, seed=77):
+    rng = np.random.default_rng(seed)
+    ncell = cfg.cpd ** 3
+    nz = np.flatnonzero(counts > 0)
+    order = nz[np.argsort(counts[nz], kind="stable")]
+    pick = set(rng.choice(ncell, size=min(n_random, ncell), replace=False).tolist())
+    pick.update(order[:n_extreme].tolist())               # sparsest non-empty cells
+    pick.update(order[-n_extreme:].tolist())              # densest cells
+    return np.array(sorted(pick), dtype=np.int32)
+
+
+FULL = [(2, 400, 8), (3, 150, 3), (4, 300, 8), (5, 60, 2)]
+
+
+@pytest.mark.parametrize("k,n_random,n_extreme", FULL, ids=[f"config{f[0]}" for f in FULL])
+def test_full_size_configs_sampled(torch_cuda, NF, oracle_mod, k, n_random, n_extreme):
+    """BASELINE.json configs at full size, in the launch configuration bench.py times: the GPU
+    result is compared with the oracle on a seeded sample of sink cells (random + the densest and
+    sparsest), and binning / pair count are verified on the full input."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[k]
+    pos = W.make_positions(cfg)
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        acc = nf.accel(torch.from_numpy(pos).cuda())
+        nf.sync()
+        pairs = nf.interaction_count()
+        dbg = nf.debug_cells()
+        got = acc.cpu().numpy()
+        del acc
+    cell, _ = oracle_mod.bin_particles(pos, cfg.cpd)
+    offsets, order = oracle_mod.cell_lists(cell, cfg.cpd)
+    assert np.array_equal(dbg["offsets"].astype(np.int64), offsets)
+    assert np.array_equal(dbg["perm"].astype(np.int64), order)
+    assert pairs == oracle_mod.pair_count(offsets, cfg.cpd, cfg.R)
+    del dbg, order
+    counts = np.diff(offsets)
+    cells = _sample_cells(cfg, counts, n_random, n_extreme)
+    ref, _ = oracle_mod.accel(pos, cfg.cpd, cfg.R, cfg.eps_p, sink_cells=cells)
+    sel = np.flatnonzero(np.isin(cell, cells))
+    assert len(sel) > 1000
+    assert np.isfinite(got).all()
+    check(got.astype(np.float64), ref, sel=sel, label=f"config {k} sample of {len(sel)} sinks")
+    # property that holds at any size: total momentum ~ 0
+    s = got.astype(np.float64)
+    assert np.abs(s.sum(0)).max() <= 1e-5 * np.abs(s).sum()
