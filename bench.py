@@ -53,7 +53,7 @@ class ClockSampler(threading.Thread):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
-        self._stop = threading.Event()
+        self._halt = threading.Event()
         self._nv = None
         try:
             import pynvml
@@ -90,15 +90,15 @@ class ClockSampler(threading.Thread):
                 self.reasons.add(nm)
 
     def run(self):
-        while not self._stop.is_set():
+        while not self._halt.is_set():
             try:
                 self._poll_nvml() if self._nv else self._poll_smi()
             except Exception:
                 pass
-            self._stop.wait(self.period)
+            self._halt.wait(self.period)
 
     def stop(self) -> dict:
-        self._stop.set()
+        self._halt.set()
         self.join(timeout=5)
         return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
@@ -238,13 +238,14 @@ def main():
         barrier()
         sampler.start()
         launches0 = nf.launch_count()
-        kernel_ms, step_ms = [], []
+        kernel_ms, step_ms, stage_acc = [], [], []
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record(stream)
         for _ in range(args.steps):
             step()
             # per-step stage events are recorded by the library on `stream`; reading them syncs
             st = nf.stage_ms()
+            stage_acc.append(st)
             kernel_ms.append(st["A5_interact_A6_unpermute"])
             step_ms.append(st["total"])
         ev1.record(stream)
@@ -310,6 +311,7 @@ def main():
             "dtype": "f32", "data": "synthetic", "config": workload,
             "sink_updates_per_s": cfg.N * world * args.steps / (total_ms * 1e-3), "pairs_per_step": pairs,
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "stage_ms": {k: statistics.mean(s[k] for s in stage_acc) for k in stage_acc[0]},
             "result_finite": acc_ok}
     print(json.dumps(line))
     if dist is not None:
