@@ -31,7 +31,8 @@ class NearFieldError(RuntimeError):
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "libnearfield_b200.so")
+    """the in-tree library, or the build named by NEARFIELD_B200_LIB (a tuning variant)"""
+    return os.environ.get("NEARFIELD_B200_LIB") or os.path.join(_HERE, "libnearfield_b200.so")
 
 
 def load_library() -> ctypes.CDLL:

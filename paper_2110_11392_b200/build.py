@@ -25,15 +25,18 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale():
+def build_library(force: bool = False, verbose: bool = False, out: str | None = None, defines: tuple = ()) -> str:
+    """Compile the library.  ``out`` / ``defines`` build a tuning variant (-DNAME=VALUE for the
+    knobs of csrc/nf_common.cuh) somewhere else; the default build is the product."""
+    lib = out or LIB
+    if force or out is not None or _stale():
         nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, "-o", LIB + ".tmp", *[os.path.join(CSRC, s) for s in SOURCES]]
+        cmd = [nvcc, *NVCC_FLAGS, *[f"-D{d}" for d in defines], "-o", lib + ".tmp", *[os.path.join(CSRC, s) for s in SOURCES]]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
-        os.replace(LIB + ".tmp", LIB)
-    return LIB
+        os.replace(lib + ".tmp", lib)
+    return lib
 
 
 if __name__ == "__main__":

@@ -124,7 +124,7 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
     if (N <= c->capN) return NF_OK;
     cudaStreamSynchronize(c->last_stream);
     free_scratch(c);
-    const int64_t capPad = ((N + c->ncell + 8 + 3) / 4) * 4 + 8;
+    const int64_t capPad = ((N + (NF_CELL_PAD - 1) * c->ncell + 8 + 3) / 4) * 4 + 8;
     const int64_t capBlk = capPad / NF_BS + c->ncol + 8;
     cudaError_t e = cudaSuccess;
     auto A = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
@@ -149,7 +149,7 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
 extern "C" nf_status nf_accel(nf_ctx *c, const float *d_pos, int64_t N, float *d_acc, void *cuda_stream) {
     if (!c) return NF_EINVAL;
     c->err[0] = 0;
-    if (N < 0 || (N > 0 && (!d_pos || !d_acc)) || (double)N + (double)c->ncell >= 2147483640.0) {
+    if (N < 0 || (N > 0 && (!d_pos || !d_acc)) || (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
         snprintf(c->err, sizeof c->err, "nf_accel: bad argument (N=%lld)", (long long)N);
         return NF_EINVAL;
     }

@@ -81,7 +81,7 @@ __device__ __forceinline__ unsigned long long block_excl_scan(unsigned long long
 // item c of the cell scan = (padded count << 32) | true count
 __device__ __forceinline__ unsigned long long cell_item(const uint32_t *counts, uint32_t c) {
     uint32_t n = counts[c];
-    return ((unsigned long long)((n + 1u) & ~1u) << 32) | n;
+    return ((unsigned long long)((n + (NF_CELL_PAD - 1u)) & ~(NF_CELL_PAD - 1u)) << 32) | n;
 }
 
 template <int MODE>   // 0: cells (from counts)  1: plain uint32 input widened to 64 bit
@@ -178,7 +178,8 @@ __global__ void __launch_bounds__(256) k_scatter(uint32_t N, const uint32_t *__r
     skey[slot] = k;
     if (r == 0) {
         uint32_t n = counts[k];
-        if (n & 1u) skey[poff[k] + n] = k | NF_PAD_FLAG;   // the padding slot of an odd cell
+        const uint32_t np = (n + (NF_CELL_PAD - 1u)) & ~(NF_CELL_PAD - 1u);
+        for (uint32_t t = n; t < np; ++t) skey[poff[k] + t] = k | NF_PAD_FLAG;   // the padding slots of the cell
     }
 }
 
@@ -235,7 +236,7 @@ nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t
     k_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_poff, ctx->d_tmp_perm, skey); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     // upper bound of the padded slot count: N + ncell (+8 slack), known on the host
-    uint64_t bound = (uint64_t)N + (uint64_t)ctx->ncell + 8;
+    uint64_t bound = (uint64_t)N + (uint64_t)(NF_CELL_PAD - 1) * (uint64_t)ctx->ncell + 8;
     if (bound > (uint64_t)ctx->capPad) bound = ctx->capPad;
     k_rank_gather<<<(uint32_t)((bound + 255) / 256), 256, 0, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl,
                                                                    ctx->d_offsets, ctx->d_poff, ctx->d_tmp_perm, ctx->d_sorted,

@@ -17,11 +17,32 @@
 #define NF_SPLINE_PER_PLUMMER 2.16  // eps_s = 2.16 eps_p
 
 // interaction kernel geometry
+#ifndef NF_NW
 #define NF_NW 4                   // consumer warps per CTA (one sink per thread)
+#endif
 #define NF_BS (NF_NW * 32)        // sinks per CTA work item
-#define NF_TILE 1024              // source slots per pipeline stage (per coordinate plane)
+#ifndef NF_TILE
+#define NF_TILE 512               // source slots per pipeline stage (per coordinate plane)
+#endif
 #define NF_TABMAX 31              // source cells per segment table (32 entries = one per producer lane)
-#define NF_NSTAGE 4               // pipeline depth
+#ifndef NF_NSTAGE
+#define NF_NSTAGE 8               // pipeline depth
+#endif
+#ifndef NF_CELL_PAD
+#define NF_CELL_PAD 2             // every cell is padded to a multiple of this many slots (power of two, >= 2)
+#endif
+#ifndef NF_UNROLL
+#define NF_UNROLL 4               // source pairs per unrolled trip of the pair loop
+#endif
+#ifndef NF_MIN_CTAS
+#define NF_MIN_CTAS 4             // resident CTAs per SM the interaction kernel is compiled for
+#endif
+#ifndef NF_PRODUCER_SLEEP_NS
+#define NF_PRODUCER_SLEEP_NS 0    // back-off of the producer warp while its ring slot is still in use
+#endif
+#ifndef NF_CONSUMER_SLEEP_NS
+#define NF_CONSUMER_SLEEP_NS 0
+#endif
 
 struct NfParams {
     int cpd, R, ncell, ncol;
@@ -55,7 +76,7 @@ struct nf_ctx {
     uint32_t *d_col_nblk, *d_col_base, *d_scan32_blk, *d_blk_order;
     NfBlockDesc *d_blk;
     uint32_t *d_ctrl;            // [0] work counter  [1] number of blocks  [2] bad-position flag  [3] npad
-                                 // [16..79] cost histogram  [96..97] float rc^2, rc  [100..101] u64 sum n_c^2
+                                 // [16..79] cost histogram  [96..98] float rc^2, rc, rc^-3  [100..101] u64 sum n_c^2
     unsigned long long *d_pairs;
     int32_t *d_nbr;              // debug neighbour list
     // host staging for nf_accel_host

@@ -31,15 +31,21 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+__device__ __forceinline__ bool mbar_try(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "NF_WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra NF_DONE_%=;\n\t"
-        "bra NF_WAIT_%=;\n\t"
-        "NF_DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
-        : "memory");
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0u;
+}
+// SLEEP_NS > 0: back off between polls so that a waiting warp does not take issue slots from
+// the working warps of its SM sub-partition (the producer is always several stages ahead).
+template <int SLEEP_NS>
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    while (!mbar_try(bar, parity)) {
+        if (SLEEP_NS > 0) __nanosleep(SLEEP_NS);
+    }
 }
 __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
@@ -148,6 +154,7 @@ __global__ void k_choose_rc(const unsigned long long *__restrict__ sum2, double 
     }
     dyn[0] = (float)(rc * rc);
     dyn[1] = (float)rc;
+    dyn[2] = rc > 0.0 ? (float)(1.0 / (rc * rc * rc)) : 0.f;   // clamp of the float32 r^-3 in near cells
 }
 
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st) {
@@ -202,74 +209,97 @@ struct InteractArgs {
     const uint32_t *skey, *poff, *perm_pad, *order;
     const NfBlockDesc *blk;
     uint32_t *ctrl;
-    const float *dyn;        // [0] rc^2 (cell units^2; 0 = no close-pair radius, use the min form)
+    const float *dyn;        // [0] rc^2 (cell units^2; 0 = no close-pair radius, use the min form)  [1] rc  [2] rc^-3
     float *acc;
     float kfac;
     NfParams prm;
 };
 
-// Exact evaluation of one close pair (r < r_c) in double precision.  The float32 cell-relative
-// offsets of the sorted planes are NOT enough here: for x < box/4 the input float32 position is
-// finer than a float32 offset of magnitude ~0.5 cell, and 1.5e-8 cell is 3e-6 of the force of a
-// pair 0.01 cell apart.  So both particles are re-read from the caller's position array through
-// the permutation and their offsets recomputed in double; the INTEGER cell shift is added last.
-// Piecewise Eq. 3.  Rare (a few per cent of the sinks have such a neighbour),
-// hence noinline and out of the hot loop.
-struct CloseCtx {
+// Close pairs (r < r_c) in double precision.  The hot loop clamps the
+// float32 r^-3 of a near cell to fmax = r_c^-3 and tracks the smallest r^2 the lane saw in that
+// cell; a lane whose minimum is below r_c^2 calls close_scan() for that one cell.  The scan
+// repeats the loop's float32 arithmetic for d and r^2 (same operations, same order, so the same
+// decision), and for every pair with r^2 < r_c^2 returns  exact F(d) d - fmax d_float,  i.e. it
+// replaces what the hot loop added by the exact value.  The float32 cell-relative offsets of
+// the sorted planes are NOT enough for the exact value: for x < box/4 the input float32 position
+// is finer than a float32 offset of magnitude ~0.5 cell, and 1.5e-8 cell is 3e-6 of the force
+// of a pair 0.01 cell apart.  So both particles are re-read from the caller's position array
+// through the permutation and their offsets recomputed in double; the INTEGER cell shift is
+// added last.  Piecewise Eq. 3.  Rare (a few per cent of the sinks have such a
+// neighbour), hence noinline and out of the hot loop.
+struct CloseArgs {
     const float *pos;          // caller's positions (input order)
     const uint32_t *perm_pad;  // padded slot -> input index
     double scale;              // cpd / box
     double eps;                // eps_s in cell units
-    uint32_t sink_slot;
-    int have_p;                // exact sink offsets cached?
-    double opx, opy, opz;      // exact sink offsets (cell units)
-    int a, b, dzc;             // integer cell shift of the source cell relative to the sink's cell
-    double sx, sy, sz;         // accumulated exact contributions
 };
 __device__ __forceinline__ double exact_offset(float x, double scale) {
     const double t = (double)x * scale;
     return t - floor(t) - 0.5;
 }
-__device__ __noinline__ void close_pair(CloseCtx &C, uint32_t src_slot) {
-    // padding slots (input index 0xffffffff) sit at +BIG: a padding SINK meets padding sources at d = 0
-    const uint32_t qi = C.perm_pad[src_slot];
-    if (qi == 0xffffffffu) return;
-    if (!C.have_p) {
-        const uint32_t pi = C.perm_pad[C.sink_slot];
-        if (pi == 0xffffffffu) return;
-        const float *p = C.pos + 3ull * pi;
-        C.opx = exact_offset(p[0], C.scale); C.opy = exact_offset(p[1], C.scale); C.opz = exact_offset(p[2], C.scale);
-        C.have_p = 1;
+__device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, const float *ys, const float *zs, int lo, int hi,
+                                        float xim, float yi, float zi, float rc2, float fmax, uint32_t g_lo, uint32_t sink_slot,
+                                        int a, int b, int dzc, double *corr /* shared: [3][NF_BS], this thread's column */) {
+    const uint32_t pi = K.perm_pad[sink_slot];
+    if (pi == 0xffffffffu) return;               // a padding sink (its result is never stored)
+    const float *p = K.pos + 3ull * pi;
+    const double opx = exact_offset(p[0], K.scale), opy = exact_offset(p[1], K.scale), opz = exact_offset(p[2], K.scale);
+    double cx = 0.0, cy = 0.0, cz = 0.0;
+    for (int s = lo; s < hi; ++s) {
+        const float dxf = __fadd_rn(xs[s], -xim), dyf = __fadd_rn(ys[s], -yi), dzf = __fadd_rn(zs[s], -zi);
+        float r2f = __fmaf_rn(dxf, dxf, NF_TAU);
+        r2f = __fmaf_rn(dyf, dyf, r2f);
+        r2f = __fmaf_rn(dzf, dzf, r2f);
+        if (!(r2f < rc2)) continue;
+        // what the hot loop added for this pair (f clamped to fmax)
+        cx -= (double)fmax * (double)dxf; cy -= (double)fmax * (double)dyf; cz -= (double)fmax * (double)dzf;
+        const uint32_t qi = K.perm_pad[g_lo + (uint32_t)s];
+        if (qi == 0xffffffffu || qi == pi) continue;      // padding never gets here (x = +BIG); self pair: F(0) = 0
+        const float *q = K.pos + 3ull * qi;
+        const double dx = (exact_offset(q[0], K.scale) - opx) + (double)a;
+        const double dy = (exact_offset(q[1], K.scale) - opy) + (double)b;
+        const double dz = (exact_offset(q[2], K.scale) - opz) + (double)dzc;
+        const double r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 == 0.0) continue;                          // coincident particles: F(0) = 0
+        const double r = sqrt(r2);
+        double f;
+        if (r < K.eps) {
+            const double u = r / K.eps;
+            f = (10.0 - 15.0 * u + 6.0 * u * u) / (K.eps * K.eps * K.eps);
+        } else {
+            f = 1.0 / (r2 * r);
+        }
+        cx += f * dx; cy += f * dy; cz += f * dz;
     }
-    const float *q = C.pos + 3ull * qi;
-    const double dx = (exact_offset(q[0], C.scale) - C.opx) + (double)C.a;
-    const double dy = (exact_offset(q[1], C.scale) - C.opy) + (double)C.b;
-    const double dz = (exact_offset(q[2], C.scale) - C.opz) + (double)C.dzc;
-    const double r2 = dx * dx + dy * dy + dz * dz;
-    if (r2 == 0.0) return;                       // self pair / coincident particles: F(0) = 0
-    const double r = sqrt(r2);
-    double f;
-    if (r < C.eps) {
-        const double u = r / C.eps;
-        f = (10.0 - 15.0 * u + 6.0 * u * u) / (C.eps * C.eps * C.eps);
-    } else {
-        f = 1.0 / (r2 * r);
-    }
-    C.sx += f * dx; C.sy += f * dy; C.sz += f * dz;
+    corr[0] += cx; corr[NF_BS] += cy; corr[2 * NF_BS] += cz;
+}
+
+__device__ __forceinline__ float fmin3(float a, float b, float c) {
+    float d;
+    asm("min.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
 }
 
 // MODE 0: far cells, pure r^-3 (11 FMA-pipe ops per pair)
-// MODE 1: near cells, Eq. 3 as min(r^-3, spline) (14 ops)            -- used when no close-pair radius is needed
-// MODE 2: near cells, r^-3 with pairs r^2 < rc2 zeroed and sent to close_pair()
-// MODE 3: as 2 for source cells that contain the sinks themselves (r^2 == 0 is not sent)
+// MODE 1: near cells, Eq. 3 as min(r^-3, spline) (14 ops)        -- used when no close-pair radius is needed
+// MODE 2: near cells, min(r^-3, r_c^-3) and the running minimum of r^2 (close pairs are fixed up by close_scan)
+// MODE 3: as 2 for the sinks' own cells: the self pair (r^2 == tau exactly, contributes 0) does not count as close
+constexpr int kUnroll = NF_UNROLL;
 template <int MODE>
 __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ zs, int lo, int hi,
                                           float xim, float yi, float zi, float2 &ax, float2 &ay, float2 &az, const float2 c0, const float2 c1,
-                                          const float2 c2, const float rc2, CloseCtx &C, const uint32_t g_lo) {
+                                          const float2 c2, const float fmax, float &m) {
     const float2 nx = make_float2(-xim, -xim), ny = make_float2(-yi, -yi), nz = make_float2(-zi, -zi);
     const float2 tau = make_float2(NF_TAU, NF_TAU);
-#pragma unroll 4
+#if NF_CELL_PAD >= 2 * NF_UNROLL
+    // cells are padded to whole unrolled trips: no remainder loop
+    for (int s0 = lo; s0 < hi; s0 += 2 * kUnroll)
+#pragma unroll
+    for (int s = s0; s < s0 + 2 * kUnroll; s += 2) {
+#else
+#pragma unroll kUnroll
     for (int s = lo; s < hi; s += 2) {
+#endif
         const float2 X = *reinterpret_cast<const float2 *>(xs + s);
         const float2 Y = *reinterpret_cast<const float2 *>(ys + s);
         const float2 Z = *reinterpret_cast<const float2 *>(zs + s);
@@ -288,13 +318,10 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
             f.y = fminf(f.y, h.y);
         }
         if (MODE >= 2) {
-            const bool p0 = r2.x < rc2, p1 = r2.y < rc2;
-            f.x = p0 ? 0.f : f.x;
-            f.y = p1 ? 0.f : f.y;
-            if (p0 | p1) {
-                if (p0 && (MODE == 2 || r2.x > 2.f * NF_TAU)) close_pair(C, g_lo + (uint32_t)s);
-                if (p1 && (MODE == 2 || r2.y > 2.f * NF_TAU)) close_pair(C, g_lo + (uint32_t)s + 1u);
-            }
+            f.x = fminf(f.x, fmax);
+            f.y = fminf(f.y, fmax);
+            if (MODE == 2) m = fmin3(m, r2.x, r2.y);
+            else m = fmin3(m, r2.x > 2.f * NF_TAU ? r2.x : NF_BIG, r2.y > 2.f * NF_TAU ? r2.y : NF_BIG);
         }
         ax = __ffma2_rn(f, dx, ax);
         ay = __ffma2_rn(f, dy, ay);
@@ -313,10 +340,11 @@ __device__ __forceinline__ void fold(float &tot, float &comp, float v, int kahan
     }
 }
 
-__global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArgs A) {
+__global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(const InteractArgs A) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Stage *stages = reinterpret_cast<Stage *>(smem_raw);
     __shared__ uint64_t full_bar[NF_NSTAGE], empty_bar[NF_NSTAGE];
+    __shared__ double close_corr[3][NF_BS];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int cpd = A.prm.cpd, R = A.prm.R;
@@ -339,7 +367,7 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
         const uint32_t nblocks = A.ctrl[1];
         auto emit = [&](int flags, int a, int b, int zu0, int nc, uint32_t tabval, uint32_t g_lo, int g_cnt, uint32_t col, uint32_t s0, uint32_t cnt) {
             Stage &S = stages[stage];
-            mbar_wait(&empty_bar[stage], phase ^ 1u);
+            mbar_wait<NF_PRODUCER_SLEEP_NS>(&empty_bar[stage], phase ^ 1u);
             S.tab[lane] = tabval;
             if (lane == 0) {
                 StageHdr h;
@@ -413,9 +441,10 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
     const int near_cheb = A.prm.near_cheb, kahan = A.prm.kahan;
     const float rc2 = A.dyn[0];
     const bool flagmode = rc2 > 0.f;
-    CloseCtx C;
-    C.pos = A.pos; C.perm_pad = A.perm_pad; C.scale = A.prm.scale; C.eps = A.prm.eps_cells;
-    C.sx = C.sy = C.sz = 0.0; C.opx = C.opy = C.opz = 0.0; C.have_p = 0; C.sink_slot = 0; C.a = C.b = C.dzc = 0;
+    const float fmax = A.dyn[2];
+    CloseArgs K;
+    K.pos = A.pos; K.perm_pad = A.perm_pad; K.scale = A.prm.scale; K.eps = A.prm.eps_cells;
+    double *corr = &close_corr[0][threadIdx.x];     // this thread's exact close-pair corrections (x, y, z)
     float px = -NF_BIG, py = 0.f, pz = 0.f;
     int zl = 0, z1 = 0, z2 = -1;
     bool valid = false, warp_active = false;
@@ -424,7 +453,7 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
 
     for (;;) {
         Stage &S = stages[stage];
-        mbar_wait(&full_bar[stage], phase);
+        mbar_wait<NF_CONSUMER_SLEEP_NS>(&full_bar[stage], phase);
         const StageHdr h = S.hdr;
         if (h.flags & NF_F_EXIT) break;
         if (h.flags & NF_F_NEWBLOCK) {
@@ -445,11 +474,10 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
                 if (!valid) zl = z2;
             }
             tx = ty = tz = kx = ky = kz = 0.f;
-            C.sink_slot = slot; C.have_p = 0; C.sx = C.sy = C.sz = 0.0;
+            corr[0] = 0.0; corr[NF_BS] = 0.0; corr[2 * NF_BS] = 0.0;
         }
         if (warp_active && h.g_cnt > 0) {
             const float xi = px - (float)h.a, yi = py - (float)h.b;
-            C.a = h.a; C.b = h.b;
             const bool near_ab = (abs(h.a) <= near_cheb) && (abs(h.b) <= near_cheb);
             int zlo = z1 - R, zhi = z2 + R;
             if (zlo < h.zu0) zlo = h.zu0;
@@ -467,11 +495,14 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
                 const float zi = pz - (float)dzc;
                 const float xim = act ? xi : -NF_BIG;   // masked sink at -BIG, padding sources at +BIG: never coincide
                 const bool near = near_ab && (zu >= z1 - near_cheb) && (zu <= z2 + near_cheb);
-                C.dzc = dzc;
-                if (!near) pair_loop<0>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, rc2, C, h.g_lo);
-                else if (!flagmode) pair_loop<1>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, rc2, C, h.g_lo);
-                else if (h.a == 0 && h.b == 0 && zu >= z1 && zu <= z2) pair_loop<3>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, rc2, C, h.g_lo);
-                else pair_loop<2>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, rc2, C, h.g_lo);
+                float m = NF_BIG;
+                if (!near) pair_loop<0>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+                else if (!flagmode) pair_loop<1>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+                else {
+                    if (h.a == 0 && h.b == 0 && zu >= z1 && zu <= z2) pair_loop<3>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+                    else pair_loop<2>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+                    if (m < rc2) close_scan(K, S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, rc2, fmax, h.g_lo, slot, h.a, h.b, dzc, corr);
+                }
             }
             fold(tx, kx, ax.x + ax.y, kahan);
             fold(ty, ky, ay.x + ay.y, kahan);
@@ -482,9 +513,9 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32) k_interact(const InteractArg
                 const uint32_t dst = A.perm_pad[slot];
                 if (dst != 0xffffffffu) {
                     float *o = A.acc + 3ull * dst;
-                    o[0] = (float)((double)A.kfac * ((double)tx + C.sx));
-                    o[1] = (float)((double)A.kfac * ((double)ty + C.sy));
-                    o[2] = (float)((double)A.kfac * ((double)tz + C.sz));
+                    o[0] = (float)((double)A.kfac * ((double)tx + corr[0]));
+                    o[1] = (float)((double)A.kfac * ((double)ty + corr[NF_BS]));
+                    o[2] = (float)((double)A.kfac * ((double)tz + corr[2 * NF_BS]));
                 }
             }
         }
