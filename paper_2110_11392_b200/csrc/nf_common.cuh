@@ -29,7 +29,7 @@
 #define NF_NSTAGE 8               // pipeline depth
 #endif
 #ifndef NF_CELL_PAD
-#define NF_CELL_PAD 2             // every cell is padded to a multiple of this many slots (power of two, >= 2)
+#define NF_CELL_PAD 4             // every cell is padded to a multiple of this many slots (power of two, >= 2)
 #endif
 #ifndef NF_UNROLL
 #define NF_UNROLL 4               // source pairs per unrolled trip of the pair loop

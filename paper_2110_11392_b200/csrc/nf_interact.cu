@@ -291,18 +291,7 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
                                           const float2 c2, const float fmax, float &m) {
     const float2 nx = make_float2(-xim, -xim), ny = make_float2(-yi, -yi), nz = make_float2(-zi, -zi);
     const float2 tau = make_float2(NF_TAU, NF_TAU);
-#if NF_CELL_PAD >= 2 * NF_UNROLL
-    // cells are padded to whole unrolled trips: no remainder loop
-    for (int s0 = lo; s0 < hi; s0 += 2 * kUnroll)
-#pragma unroll
-    for (int s = s0; s < s0 + 2 * kUnroll; s += 2) {
-#else
-#pragma unroll kUnroll
-    for (int s = lo; s < hi; s += 2) {
-#endif
-        const float2 X = *reinterpret_cast<const float2 *>(xs + s);
-        const float2 Y = *reinterpret_cast<const float2 *>(ys + s);
-        const float2 Z = *reinterpret_cast<const float2 *>(zs + s);
+    auto pair2 = [&](const float2 X, const float2 Y, const float2 Z) {
         const float2 dx = __fadd2_rn(X, nx), dy = __fadd2_rn(Y, ny), dz = __fadd2_rn(Z, nz);
         float2 r2 = __ffma2_rn(dx, dx, tau);
         r2 = __ffma2_rn(dy, dy, r2);
@@ -326,7 +315,23 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
         ax = __ffma2_rn(f, dx, ax);
         ay = __ffma2_rn(f, dy, ay);
         az = __ffma2_rn(f, dz, az);
+    };
+#if NF_CELL_PAD >= 4
+    // cells start on 16-byte boundaries: four sources per LDS.128, two such quads per trip
+#pragma unroll 2
+    for (int s = lo; s < hi; s += 4) {
+        const float4 X = *reinterpret_cast<const float4 *>(xs + s);
+        const float4 Y = *reinterpret_cast<const float4 *>(ys + s);
+        const float4 Z = *reinterpret_cast<const float4 *>(zs + s);
+        pair2(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y));
+        pair2(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w));
     }
+#else
+#pragma unroll kUnroll
+    for (int s = lo; s < hi; s += 2) {
+        pair2(*reinterpret_cast<const float2 *>(xs + s), *reinterpret_cast<const float2 *>(ys + s), *reinterpret_cast<const float2 *>(zs + s));
+    }
+#endif
 }
 
 __device__ __forceinline__ void fold(float &tot, float &comp, float v, int kahan) {
