@@ -135,7 +135,7 @@ nf_status nf_stage_ms(nf_ctx *ctx, float *h_ms /* NF_N_STAGES */);
  *                                  ascending input index within a cell (stable).
  *   *d_sorted   float[4][Npad]     four planes (x, y, z offsets from the cell centre in CELL
  *                                  units, then the cell key as uint32) in PADDED slot order;
- *   *d_poffsets uint32[cpd^3 + 1]  first padded slot of each cell (cells padded to even size)
+ *   *d_poffsets uint32[cpd^3 + 1]  first padded slot of each cell (cells padded to a multiple of 4 slots)
  * Any out-pointer may be NULL.
  */
 nf_status nf_debug_cells(nf_ctx *ctx, const uint32_t **d_offsets, const uint32_t **d_perm,

@@ -18,24 +18,29 @@
 
 // interaction kernel geometry
 #ifndef NF_NW
-#define NF_NW 4                   // consumer warps per CTA (one sink per thread)
+#define NF_NW 4                   // consumer warps per CTA
 #endif
-#define NF_BS (NF_NW * 32)        // sinks per CTA work item
+#ifndef NF_SINKS
+#define NF_SINKS 2                // sinks per consumer thread (adjacent slots 2t, 2t+1 of the warp's range when 2)
+#endif
+#define NF_BS (NF_NW * 32 * NF_SINKS)   // sinks per CTA work item
+#ifndef NF_QUADS_PER_TRIP
+#define NF_QUADS_PER_TRIP 2   // source quads per unrolled trip of the pair loop
+#endif
 #ifndef NF_TILE
-#define NF_TILE 512               // source slots per pipeline stage (per coordinate plane)
+#define NF_TILE 640               // source slots per pipeline stage (per coordinate plane)
 #endif
 #define NF_TABMAX 31              // source cells per segment table (32 entries = one per producer lane)
 #ifndef NF_NSTAGE
-#define NF_NSTAGE 8               // pipeline depth
+#define NF_NSTAGE 7               // pipeline depth
 #endif
 #ifndef NF_CELL_PAD
 #define NF_CELL_PAD 4             // every cell is padded to a multiple of this many slots (power of two, >= 2)
 #endif
 #ifndef NF_UNROLL
-#define NF_UNROLL 4               // source pairs per unrolled trip of the pair loop
 #endif
 #ifndef NF_MIN_CTAS
-#define NF_MIN_CTAS 4             // resident CTAs per SM the interaction kernel is compiled for
+#define NF_MIN_CTAS 3             // resident CTAs per SM the interaction kernel is compiled for
 #endif
 #ifndef NF_PRODUCER_SLEEP_NS
 #define NF_PRODUCER_SLEEP_NS 0    // back-off of the producer warp while its ring slot is still in use

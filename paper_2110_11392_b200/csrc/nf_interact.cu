@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(128) k_fill_blocks(int ncol, int cpd, const ui
     const uint32_t nb = col_nblk[col];
     if (nb == 0) return;
     const uint32_t p0 = poff[col * cpd], n = poff[(col + 1) * cpd] - p0;
-    const uint32_t bs = (((n + nb - 1) / nb) + 31u) & ~31u;
+    const uint32_t bs = (((n + nb - 1) / nb) + (32u * NF_SINKS - 1u)) & ~(32u * NF_SINKS - 1u);
     const uint32_t base = col_base[col];
     // cost estimate: sinks x (sources of the whole home column window), cheap proxy = sinks x column density x (2R+1+span)
     for (uint32_t k = 0; k < nb; ++k) {
@@ -284,15 +284,22 @@ __device__ __forceinline__ float fmin3(float a, float b, float c) {
 // MODE 1: near cells, Eq. 3 as min(r^-3, spline) (14 ops)        -- used when no close-pair radius is needed
 // MODE 2: near cells, min(r^-3, r_c^-3) and the running minimum of r^2 (close pairs are fixed up by close_scan)
 // MODE 3: as 2 for the sinks' own cells: the self pair (r^2 == tau exactly, contributes 0) does not count as close
-constexpr int kUnroll = NF_UNROLL;
+// Sources [lo, lo + n) of the stage (lo may differ between lanes, n is warp-uniform and a
+// multiple of 4; cells start on 16-byte boundaries) against the NF_SINKS sinks of this thread:
+// four sources per LDS.128 and plane, shared by the thread's sinks.
+constexpr int kS = NF_SINKS;
+constexpr int kQuads = NF_QUADS_PER_TRIP;
 template <int MODE>
-__device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ zs, int lo, int hi,
-                                          float xim, float yi, float zi, float2 &ax, float2 &ay, float2 &az, const float2 c0, const float2 c1,
-                                          const float2 c2, const float fmax, float &m) {
-    const float2 nx = make_float2(-xim, -xim), ny = make_float2(-yi, -yi), nz = make_float2(-zi, -zi);
+__device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ zs, int lo, int n,
+                                          const float (&xim)[kS], const float (&yi)[kS], const float (&zi)[kS], float2 (&ax)[kS],
+                                          float2 (&ay)[kS], float2 (&az)[kS], const float2 c0, const float2 c1, const float2 c2,
+                                          const float fmax, float (&m)[kS]) {
     const float2 tau = make_float2(NF_TAU, NF_TAU);
-    auto pair2 = [&](const float2 X, const float2 Y, const float2 Z) {
-        const float2 dx = __fadd2_rn(X, nx), dy = __fadd2_rn(Y, ny), dz = __fadd2_rn(Z, nz);
+    float2 nx[kS], ny[kS], nz[kS];
+#pragma unroll
+    for (int j = 0; j < kS; ++j) { nx[j] = make_float2(-xim[j], -xim[j]); ny[j] = make_float2(-yi[j], -yi[j]); nz[j] = make_float2(-zi[j], -zi[j]); }
+    auto pair2 = [&](const int j, const float2 X, const float2 Y, const float2 Z) {
+        const float2 dx = __fadd2_rn(X, nx[j]), dy = __fadd2_rn(Y, ny[j]), dz = __fadd2_rn(Z, nz[j]);
         float2 r2 = __ffma2_rn(dx, dx, tau);
         r2 = __ffma2_rn(dy, dy, r2);
         r2 = __ffma2_rn(dz, dz, r2);
@@ -309,29 +316,25 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
         if (MODE >= 2) {
             f.x = fminf(f.x, fmax);
             f.y = fminf(f.y, fmax);
-            if (MODE == 2) m = fmin3(m, r2.x, r2.y);
-            else m = fmin3(m, r2.x > 2.f * NF_TAU ? r2.x : NF_BIG, r2.y > 2.f * NF_TAU ? r2.y : NF_BIG);
+            if (MODE == 2) m[j] = fmin3(m[j], r2.x, r2.y);
+            else m[j] = fmin3(m[j], r2.x > 2.f * NF_TAU ? r2.x : NF_BIG, r2.y > 2.f * NF_TAU ? r2.y : NF_BIG);
         }
-        ax = __ffma2_rn(f, dx, ax);
-        ay = __ffma2_rn(f, dy, ay);
-        az = __ffma2_rn(f, dz, az);
+        ax[j] = __ffma2_rn(f, dx, ax[j]);
+        ay[j] = __ffma2_rn(f, dy, ay[j]);
+        az[j] = __ffma2_rn(f, dz, az[j]);
     };
-#if NF_CELL_PAD >= 4
-    // cells start on 16-byte boundaries: four sources per LDS.128, two such quads per trip
-#pragma unroll 2
-    for (int s = lo; s < hi; s += 4) {
-        const float4 X = *reinterpret_cast<const float4 *>(xs + s);
-        const float4 Y = *reinterpret_cast<const float4 *>(ys + s);
-        const float4 Z = *reinterpret_cast<const float4 *>(zs + s);
-        pair2(make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y));
-        pair2(make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w));
+    const float *px = xs + lo, *py = ys + lo, *pz = zs + lo;
+#pragma unroll kQuads
+    for (int t = 0; t < n; t += 4) {
+        const float4 X = *reinterpret_cast<const float4 *>(px + t);
+        const float4 Y = *reinterpret_cast<const float4 *>(py + t);
+        const float4 Z = *reinterpret_cast<const float4 *>(pz + t);
+#pragma unroll
+        for (int j = 0; j < kS; ++j) {
+            pair2(j, make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y));
+            pair2(j, make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w));
+        }
     }
-#else
-#pragma unroll kUnroll
-    for (int s = lo; s < hi; s += 2) {
-        pair2(*reinterpret_cast<const float2 *>(xs + s), *reinterpret_cast<const float2 *>(ys + s), *reinterpret_cast<const float2 *>(zs + s));
-    }
-#endif
 }
 
 __device__ __forceinline__ void fold(float &tot, float &comp, float v, int kahan) {
@@ -345,11 +348,17 @@ __device__ __forceinline__ void fold(float &tot, float &comp, float v, int kahan
     }
 }
 
+// FLAG = the regime k_choose_rc picked on the device: true = a close-pair radius is in use
+// (near cells: clamp + close_scan), false = Eq. 3 as a min in near cells.  Both instantiations
+// are launched; the one whose regime is not in force returns at once (no host round trip).
+template <bool FLAG>
 __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(const InteractArgs A) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Stage *stages = reinterpret_cast<Stage *>(smem_raw);
     __shared__ uint64_t full_bar[NF_NSTAGE], empty_bar[NF_NSTAGE];
     __shared__ double close_corr[3][NF_BS];
+    __shared__ float tot[6][NF_BS];      // per sink: running sums x, y, z and their Kahan compensations
+    if ((A.dyn[0] > 0.f) != FLAG) return;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int cpd = A.prm.cpd, R = A.prm.R;
@@ -427,7 +436,13 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
                             const uint32_t gl = g0 & ~3u, ge = (g1 + 3u) & ~3u;
                             for (uint32_t c0 = gl; c0 < ge; c0 += NF_TILE) {
                                 const uint32_t c1 = (c0 + NF_TILE < ge) ? c0 + NF_TILE : ge;
-                                emit(flags, a, b, u, run, tv, c0, (int)(c1 - c0), d.col, d.s0, d.cnt);
+                                {
+                                    // table entry = first slot of the cell relative to this stage, clamped to the stage
+                                    int tl = (int)(tv - c0);
+                                    const int tc = (int)(c1 - c0);
+                                    tl = tl < 0 ? 0 : (tl > tc ? tc : tl);
+                                    emit(flags, a, b, u, run, (uint32_t)tl, c0, tc, d.col, d.s0, d.cnt);
+                                }
                                 flags = 0;
                             }
                         }
@@ -442,85 +457,141 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
     }
 
     // =============================== consumer warps ==========================================
+    // Thread t of warp w holds the kS sinks at slots s0 + (32 w + t) kS + j of the block (adjacent
+    // slots: cells are padded to 4 slots and blocks start on multiples of 4, so they share a cell).
     const float2 c0 = make_float2(A.prm.c0, A.prm.c0), c1 = make_float2(A.prm.c1, A.prm.c1), c2 = make_float2(A.prm.c2, A.prm.c2);
     const int near_cheb = A.prm.near_cheb, kahan = A.prm.kahan;
     const float rc2 = A.dyn[0];
-    const bool flagmode = rc2 > 0.f;
     const float fmax = A.dyn[2];
     CloseArgs K;
     K.pos = A.pos; K.perm_pad = A.perm_pad; K.scale = A.prm.scale; K.eps = A.prm.eps_cells;
-    double *corr = &close_corr[0][threadIdx.x];     // this thread's exact close-pair corrections (x, y, z)
-    float px = -NF_BIG, py = 0.f, pz = 0.f;
+    const int tid_s = (int)threadIdx.x * kS;           // this thread's first column of close_corr / tot
+    float px[kS], py[kS], pz[kS];
+#pragma unroll
+    for (int j = 0; j < kS; ++j) { px[j] = -NF_BIG; py[j] = 0.f; pz[j] = 0.f; }
     int zl = 0, z1 = 0, z2 = -1;
-    bool valid = false, warp_active = false;
+    bool valid = false;
     uint32_t slot = 0;
-    float tx = 0.f, ty = 0.f, tz = 0.f, kx = 0.f, ky = 0.f, kz = 0.f;
+    const int W = 2 * R + 1;
 
     for (;;) {
         Stage &S = stages[stage];
         mbar_wait<NF_CONSUMER_SLEEP_NS>(&full_bar[stage], phase);
-        const StageHdr h = S.hdr;
-        if (h.flags & NF_F_EXIT) break;
-        if (h.flags & NF_F_NEWBLOCK) {
-            const uint32_t off = (uint32_t)(warp * 32 + lane);
-            valid = off < h.cnt;
-            slot = h.s0 + (valid ? off : 0u);
-            const int colbase = (int)h.col * cpd;
-            const uint32_t k = A.skey[slot];
-            zl = (int)(k & ~NF_PAD_FLAG) - colbase;
-            px = valid ? A.sx[slot] : -NF_BIG;
-            py = A.sy[slot];
-            pz = A.sz[slot];
+        const int flags = S.hdr.flags;
+        if (flags & NF_F_EXIT) break;
+        if (flags & NF_F_NEWBLOCK) {
+            const uint32_t off = (uint32_t)(warp * 32 + lane) * kS;
+            valid = off < S.hdr.cnt;
+            slot = S.hdr.s0 + (valid ? off : 0u);
+            const int colbase = (int)S.hdr.col * cpd;
+            zl = (int)(A.skey[slot] & ~NF_PAD_FLAG) - colbase;
+#pragma unroll
+            for (int j = 0; j < kS; ++j) {
+                px[j] = valid ? A.sx[slot + j] : -NF_BIG;   // an idle lane sits at -BIG: contributes and receives exactly 0
+                py[j] = A.sy[slot + j];
+                pz[j] = A.sz[slot + j];
+            }
             const unsigned vm = __ballot_sync(0xffffffffu, valid);
-            warp_active = vm != 0u;
-            if (warp_active) {
+            z1 = 0; z2 = -4 * NF_MAX_R - 4;          // no valid sink in this warp: empty z range for every stage
+            if (vm != 0u) {
                 z1 = __shfl_sync(0xffffffffu, zl, 0);
                 z2 = __shfl_sync(0xffffffffu, zl, 31 - __clz(vm));
                 if (!valid) zl = z2;
             }
-            tx = ty = tz = kx = ky = kz = 0.f;
-            corr[0] = 0.0; corr[NF_BS] = 0.0; corr[2 * NF_BS] = 0.0;
+#pragma unroll
+            for (int j = 0; j < kS; ++j) {
+#pragma unroll
+                for (int q = 0; q < 6; ++q) tot[q][tid_s + j] = 0.f;
+#pragma unroll
+                for (int q = 0; q < 3; ++q) close_corr[q][tid_s + j] = 0.0;
+            }
         }
-        if (warp_active && h.g_cnt > 0) {
-            const float xi = px - (float)h.a, yi = py - (float)h.b;
-            const bool near_ab = (abs(h.a) <= near_cheb) && (abs(h.b) <= near_cheb);
-            int zlo = z1 - R, zhi = z2 + R;
-            if (zlo < h.zu0) zlo = h.zu0;
-            if (zhi > h.zu0 + h.nc - 1) zhi = h.zu0 + h.nc - 1;
-            float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax;
-            const uint32_t g_hi = h.g_lo + (uint32_t)h.g_cnt;
-            for (int zu = zlo; zu <= zhi; ++zu) {
-                uint32_t t0 = S.tab[zu - h.zu0], t1 = S.tab[zu - h.zu0 + 1];
-                if (t0 < h.g_lo) t0 = h.g_lo;
-                if (t1 > g_hi) t1 = g_hi;
-                if (t0 >= t1) continue;
-                const int lo = (int)(t0 - h.g_lo), hi = (int)(t1 - h.g_lo);
-                const int dzc = zu - zl;
-                const bool act = valid && (abs(dzc) <= R);
-                const float zi = pz - (float)dzc;
-                const float xim = act ? xi : -NF_BIG;   // masked sink at -BIG, padding sources at +BIG: never coincide
-                const bool near = near_ab && (zu >= z1 - near_cheb) && (zu <= z2 + near_cheb);
-                float m = NF_BIG;
-                if (!near) pair_loop<0>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
-                else if (!flagmode) pair_loop<1>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+        const int zu0 = S.hdr.zu0;
+        int cz0 = z1 - R, cz1 = z2 + R;              // source cells this warp needs ...
+        if (cz0 < zu0) cz0 = zu0;
+        if (cz1 > zu0 + S.hdr.nc - 1) cz1 = zu0 + S.hdr.nc - 1;   // ... that this stage holds
+        if (S.hdr.g_cnt > 0 && cz0 <= cz1) {
+            const int ha = S.hdr.a, hb = S.hdr.b;
+            float xi[kS], yi[kS];
+#pragma unroll
+            for (int j = 0; j < kS; ++j) { xi[j] = px[j] - (float)ha; yi[j] = py[j] - (float)hb; }
+            // near cells: may hold r < eps_s; home cells: the sinks' own cells (self pairs)
+            int nz0 = 1 << 30, nz1 = -(1 << 30), hz0 = 1 << 30, hz1 = -(1 << 30);
+            if (abs(ha) <= near_cheb && abs(hb) <= near_cheb) { nz0 = z1 - near_cheb; nz1 = z2 + near_cheb; }
+            if (ha == 0 && hb == 0) { hz0 = z1; hz1 = z2; }
+            auto mode_of = [&](int zu) { return (zu < nz0 || zu > nz1) ? 0 : (!FLAG ? 1 : ((zu >= hz0 && zu <= hz1) ? 3 : 2)); };
+            const int *tab = reinterpret_cast<const int *>(S.tab) - zu0;   // tab[zu] = first stage-local slot of source cell zu
+            float2 ax[kS], ay[kS], az[kS];
+#pragma unroll
+            for (int j = 0; j < kS; ++j) { ax[j] = make_float2(0.f, 0.f); ay[j] = ax[j]; az[j] = ax[j]; }
+
+            // One pass = sources [lo, lo + n) where a lane reads cell cA's part (from loA) if its
+            // sink is within R cells of cA, else cell cB's part (from loB) if within R of cB, else
+            // it is masked.  cB = cA + 2R+1, so the two lane groups are disjoint: the edge cells
+            // of the warp's window, each needed by only part of the warp, are processed two at a
+            // time and no lane idles.
+            auto pass = [&](int loA, int cA, int loB, int cB, int n, int mode) {
+                const bool useA = abs(zl - cA) <= R, useB = abs(zl - cB) <= R;
+                const int cell = useA ? cA : cB;
+                const int lo = useA ? loA : loB;
+                const int dzc = cell - zl;
+                float xim[kS], zi[kS], m[kS];
+#pragma unroll
+                for (int j = 0; j < kS; ++j) {
+                    xim[j] = (useA || useB) ? xi[j] : -NF_BIG;    // masked sink at -BIG, padding sources at +BIG: never coincide
+                    zi[j] = pz[j] - (float)dzc;
+                    m[j] = NF_BIG;
+                }
+                if (mode == 0) pair_loop<0>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+                else if (!FLAG) pair_loop<1>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
                 else {
-                    if (h.a == 0 && h.b == 0 && zu >= z1 && zu <= z2) pair_loop<3>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
-                    else pair_loop<2>(S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
-                    if (m < rc2) close_scan(K, S.xs, S.ys, S.zs, lo, hi, xim, yi, zi, rc2, fmax, h.g_lo, slot, h.a, h.b, dzc, corr);
+                    if (mode == 3) pair_loop<3>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+                    else pair_loop<2>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+#pragma unroll
+                    for (int j = 0; j < kS; ++j)
+                        if (m[j] < rc2)
+                            close_scan(K, S.xs, S.ys, S.zs, lo, lo + n, xim[j], yi[j], zi[j], rc2, fmax, S.hdr.g_lo, slot + j, ha, hb, dzc,
+                                       &close_corr[0][tid_s + j]);
+                }
+            };
+            // cells cz0 + i with (i div W) even are "A" cells; each takes the cell W further on as partner
+            for (int base = cz0; base <= cz1; base += 2 * W) {
+                const int lastA = (base + W - 1 < cz1) ? base + W - 1 : cz1;
+                for (int cA = base; cA <= lastA; ++cA) {
+                    const int cB = cA + W;
+                    const int a0 = tab[cA], a1 = tab[cA + 1];
+                    int b0 = 0, b1 = 0;
+                    int mA = mode_of(cA), mB = 0;
+                    if (cB <= cz1) { b0 = tab[cB]; b1 = tab[cB + 1]; mB = mode_of(cB); }
+                    const int nA = a1 - a0, nB = b1 - b0;
+                    const int ncm = nA < nB ? nA : nB;
+                    if (ncm > 0) pass(a0, cA, b0, cB, ncm, mA > mB ? mA : mB);
+                    if (nA > ncm) pass(a0 + ncm, cA, 0, -(1 << 28), nA - ncm, mA);          // rest of the longer cell: its own lanes only
+                    else if (nB > ncm) pass(b0 + ncm, cB, 0, -(1 << 28), nB - ncm, mB);
                 }
             }
-            fold(tx, kx, ax.x + ax.y, kahan);
-            fold(ty, ky, ay.x + ay.y, kahan);
-            fold(tz, kz, az.x + az.y, kahan);
+#pragma unroll
+            for (int j = 0; j < kS; ++j) {
+                const float v[3] = {ax[j].x + ax[j].y, ay[j].x + ay[j].y, az[j].x + az[j].y};
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    float t = tot[q][tid_s + j], c = tot[q + 3][tid_s + j];
+                    fold(t, c, v[q], kahan);
+                    tot[q][tid_s + j] = t; tot[q + 3][tid_s + j] = c;
+                }
+            }
         }
-        if (h.flags & NF_F_LAST) {
+        if (flags & NF_F_LAST) {
             if (valid) {
-                const uint32_t dst = A.perm_pad[slot];
-                if (dst != 0xffffffffu) {
-                    float *o = A.acc + 3ull * dst;
-                    o[0] = (float)((double)A.kfac * ((double)tx + corr[0]));
-                    o[1] = (float)((double)A.kfac * ((double)ty + corr[NF_BS]));
-                    o[2] = (float)((double)A.kfac * ((double)tz + corr[2 * NF_BS]));
+#pragma unroll
+                for (int j = 0; j < kS; ++j) {
+                    const uint32_t dst = A.perm_pad[slot + j];
+                    if (dst != 0xffffffffu) {
+                        float *o = A.acc + 3ull * dst;
+                        o[0] = (float)((double)A.kfac * ((double)tot[0][tid_s + j] + close_corr[0][tid_s + j]));
+                        o[1] = (float)((double)A.kfac * ((double)tot[1][tid_s + j] + close_corr[1][tid_s + j]));
+                        o[2] = (float)((double)A.kfac * ((double)tot[2][tid_s + j] + close_corr[2][tid_s + j]));
+                    }
                 }
             }
         }
@@ -534,9 +605,13 @@ static int g_interact_blocks_per_sm = 0;
 
 nf_status nf_interact_setup(nf_ctx *ctx) {
     const size_t smem = sizeof(Stage) * NF_NSTAGE;
-    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_interact, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_interact<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_interact<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_interact, (NF_NW + 1) * 32, smem));
+    NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_interact<true>, (NF_NW + 1) * 32, smem));
+    int nb2 = 0;
+    NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb2, k_interact<false>, (NF_NW + 1) * 32, smem));
+    if (nb2 < nb) nb = nb2;
     if (nb < 1) { snprintf(ctx->err, sizeof(ctx->err), "interaction kernel does not fit on an SM"); return NF_ECUDA; }
     g_interact_blocks_per_sm = nb;
     return NF_OK;
@@ -551,7 +626,8 @@ nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_a
     A.ctrl = ctx->d_ctrl; A.dyn = (const float *)(ctx->d_ctrl + 96); A.acc = d_acc; A.kfac = kfac; A.prm = ctx->prm;
     A.prm.kahan = ctx->opt_kahan;
     const int grid = ctx->sm_count * g_interact_blocks_per_sm;
-    k_interact<<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
+    k_interact<true><<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
+    k_interact<false><<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }
