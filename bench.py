@@ -46,6 +46,25 @@ def _peaks():
         return {}
 
 
+def _ncu_traffic(config: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one k_interact launch, from the newest committed
+    ``ncu --set full`` summary of this workload under profiles/ (text; None if there is none)."""
+    import glob
+    import re
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_k_interact_cfg{config}.txt"))):
+        tot, n = 0.0, 0
+        with open(path) as f:
+            for line in f:
+                m = re.match(r"dram__bytes_(read|write)\.sum\s+([0-9.]+)\s+(\w+)", line)
+                if m:
+                    tot += float(m.group(2)) * {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}.get(m.group(3), 1.0)
+                    n += 1
+        if n == 2:
+            best = (tot, os.path.relpath(path, ROOT))
+    return best
+
+
 class ClockSampler(threading.Thread):
     """samples SM clock + throttle reasons during the timed region (pynvml, else nvidia-smi)."""
 
@@ -287,10 +306,13 @@ def main():
     n_sm = peaks_live["sm_count"]
     peak_lane = n_sm * 128 * sm_max * 1e6                   # FP32 FMA lanes x clock
     k_ms = statistics.mean(kernel_ms)
+    traffic = _ncu_traffic(args.config)
     ach_lane = pairs * FMA_LANE_OPS_PER_PAIR / (k_ms * 1e-3)
     roofline = {"bound": "alu", "kernel": "k_interact (A5 + fused A6)",
                 "achieved": ach_lane * 2 / 1e12, "peak": peak_lane * 2 / 1e12, "unit": "TFLOP/s",
-                "frac": ach_lane / peak_lane, "traffic": None,
+                "frac": ach_lane / peak_lane, "traffic": traffic[0] if traffic else None,
+                "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
+                "traffic_source": traffic[1] if traffic else None,
                 "convention": f"{FMA_LANE_OPS_PER_PAIR} FP32 FMA-pipe lane-ops per pair x 2 flop (SURVEY.md 8(a) note 2); "
                               f"peak = {n_sm} SMs x 128 lanes x {sm_max:.0f} MHz x 2 (derived, DESIGN.md); "
                               f"{FLOP_PER_PAIR} flop/pair convention -> {pairs * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12:.1f} TFLOP/s",

@@ -41,7 +41,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     c->device = dev; c->cpd = cpd; c->R = R; c->eps_p = eps_plummer; c->box = box; c->gm = 0.0;
     c->sm_count = prop.multiProcessorCount;
     c->ncell = (int64_t)cpd * cpd * cpd; c->ncol = (int64_t)cpd * cpd;
-    c->opt_kahan = 1; c->opt_heavy_first = 1; c->opt_stage_timing = 0; c->opt_rc = -1.f;
+    c->opt_kahan = 1; c->opt_heavy_first = 0; c->opt_stage_timing = 0; c->opt_rc = -1.f;
     NfParams &p = c->prm;
     p.cpd = cpd; p.R = R; p.ncell = (int)c->ncell; p.ncol = (int)c->ncol;
     p.scale = (double)cpd / box;

@@ -25,7 +25,7 @@
 #endif
 #define NF_BS (NF_NW * 32 * NF_SINKS)   // sinks per CTA work item
 #ifndef NF_QUADS_PER_TRIP
-#define NF_QUADS_PER_TRIP 2   // source quads per unrolled trip of the pair loop
+#define NF_QUADS_PER_TRIP 2     // source quads per unrolled trip of the pair loop (1 or 2)
 #endif
 #ifndef NF_TILE
 #define NF_TILE 640               // source slots per pipeline stage (per coordinate plane)

@@ -238,6 +238,7 @@ __device__ __forceinline__ double exact_offset(float x, double scale) {
     return t - floor(t) - 0.5;
 }
 __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, const float *ys, const float *zs, int lo, int hi,
+                                        uint32_t bits, int seg /* sources per flagged segment */,
                                         float xim, float yi, float zi, float rc2, float fmax, uint32_t g_lo, uint32_t sink_slot,
                                         int a, int b, int dzc, double *corr /* shared: [3][NF_BS], this thread's column */) {
     const uint32_t pi = K.perm_pad[sink_slot];
@@ -245,7 +246,12 @@ __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, con
     const float *p = K.pos + 3ull * pi;
     const double opx = exact_offset(p[0], K.scale), opy = exact_offset(p[1], K.scale), opz = exact_offset(p[2], K.scale);
     double cx = 0.0, cy = 0.0, cz = 0.0;
-    for (int s = lo; s < hi; ++s) {
+    while (bits) {
+    const int bit = __ffs(bits) - 1;
+    bits &= bits - 1u;
+    const int s0 = lo + bit * seg;
+    const int s1 = (s0 + seg < hi) ? s0 + seg : hi;
+    for (int s = s0; s < s1; ++s) {
         const float dxf = __fadd_rn(xs[s], -xim), dyf = __fadd_rn(ys[s], -yi), dzf = __fadd_rn(zs[s], -zi);
         float r2f = __fmaf_rn(dxf, dxf, NF_TAU);
         r2f = __fmaf_rn(dyf, dyf, r2f);
@@ -271,6 +277,7 @@ __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, con
         }
         cx += f * dx; cy += f * dy; cz += f * dz;
     }
+    }
     corr[0] += cx; corr[NF_BS] += cy; corr[2 * NF_BS] += cz;
 }
 
@@ -289,15 +296,17 @@ __device__ __forceinline__ float fmin3(float a, float b, float c) {
 // four sources per LDS.128 and plane, shared by the thread's sinks.
 constexpr int kS = NF_SINKS;
 constexpr int kQuads = NF_QUADS_PER_TRIP;
-template <int MODE>
+constexpr int kShortPass = 96;                       // passes up to this many sources flag close pairs per pass, longer ones per trip
+template <int MODE, bool TRIPBITS>
 __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ zs, int lo, int n,
                                           const float (&xim)[kS], const float (&yi)[kS], const float (&zi)[kS], float2 (&ax)[kS],
                                           float2 (&ay)[kS], float2 (&az)[kS], const float2 c0, const float2 c1, const float2 c2,
-                                          const float fmax, float (&m)[kS]) {
+                                          const float fmax, const float rc2, const int sh, uint32_t (&bits)[kS]) {
     const float2 tau = make_float2(NF_TAU, NF_TAU);
     float2 nx[kS], ny[kS], nz[kS];
 #pragma unroll
     for (int j = 0; j < kS; ++j) { nx[j] = make_float2(-xim[j], -xim[j]); ny[j] = make_float2(-yi[j], -yi[j]); nz[j] = make_float2(-zi[j], -zi[j]); }
+    float m[kS];
     auto pair2 = [&](const int j, const float2 X, const float2 Y, const float2 Z) {
         const float2 dx = __fadd2_rn(X, nx[j]), dy = __fadd2_rn(Y, ny[j]), dz = __fadd2_rn(Z, nz[j]);
         float2 r2 = __ffma2_rn(dx, dx, tau);
@@ -324,8 +333,7 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
         az[j] = __ffma2_rn(f, dz, az[j]);
     };
     const float *px = xs + lo, *py = ys + lo, *pz = zs + lo;
-#pragma unroll kQuads
-    for (int t = 0; t < n; t += 4) {
+    auto quad = [&](const int t) {
         const float4 X = *reinterpret_cast<const float4 *>(px + t);
         const float4 Y = *reinterpret_cast<const float4 *>(py + t);
         const float4 Z = *reinterpret_cast<const float4 *>(pz + t);
@@ -334,6 +342,44 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
             pair2(j, make_float2(X.x, X.y), make_float2(Y.x, Y.y), make_float2(Z.x, Z.y));
             pair2(j, make_float2(X.z, X.w), make_float2(Y.z, Y.w), make_float2(Z.z, Z.w));
         }
+    };
+    // A trip = kQuads source quads.  In modes 2/3 the loop records, per sink, where it saw a
+    // close pair, so that close_scan revisits only those sources: TRIPBITS (long passes) sets
+    // bit (trip >> sh) of `bits` after every trip (at most 32 segments per pass); short passes
+    // keep one running minimum and flag the whole pass (bit 0).
+    const int nfull = n / (4 * kQuads);
+    if (MODE >= 2 && !TRIPBITS) {
+#pragma unroll
+        for (int j = 0; j < kS; ++j) m[j] = NF_BIG;
+    }
+    int trip = 0;
+    for (; trip < nfull; ++trip) {
+        const int t = trip * (4 * kQuads);
+        if (MODE >= 2 && TRIPBITS) {
+#pragma unroll
+            for (int j = 0; j < kS; ++j) m[j] = NF_BIG;
+        }
+#pragma unroll
+        for (int q = 0; q < kQuads; ++q) quad(t + 4 * q);
+        if (MODE >= 2 && TRIPBITS) {
+#pragma unroll
+            for (int j = 0; j < kS; ++j) bits[j] |= (m[j] < rc2 ? 1u : 0u) << (trip >> sh);
+        }
+    }
+    if (kQuads == 2 && (n & 4)) {
+        if (MODE >= 2 && TRIPBITS) {
+#pragma unroll
+            for (int j = 0; j < kS; ++j) m[j] = NF_BIG;
+        }
+        quad(trip * 8);
+        if (MODE >= 2 && TRIPBITS) {
+#pragma unroll
+            for (int j = 0; j < kS; ++j) bits[j] |= (m[j] < rc2 ? 1u : 0u) << (trip >> sh);
+        }
+    }
+    if (MODE >= 2 && !TRIPBITS) {
+#pragma unroll
+        for (int j = 0; j < kS; ++j) bits[j] = m[j] < rc2 ? 1u : 0u;
     }
 }
 
@@ -535,22 +581,32 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
                 const int cell = useA ? cA : cB;
                 const int lo = useA ? loA : loB;
                 const int dzc = cell - zl;
-                float xim[kS], zi[kS], m[kS];
+                float xim[kS], zi[kS];
+                uint32_t bits[kS];
 #pragma unroll
                 for (int j = 0; j < kS; ++j) {
                     xim[j] = (useA || useB) ? xi[j] : -NF_BIG;    // masked sink at -BIG, padding sources at +BIG: never coincide
                     zi[j] = pz[j] - (float)dzc;
-                    m[j] = NF_BIG;
+                    bits[j] = 0u;
                 }
-                if (mode == 0) pair_loop<0>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
-                else if (!FLAG) pair_loop<1>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+                if (mode == 0) pair_loop<0, false>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits);
+                else if (!FLAG) pair_loop<1, false>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits);
                 else {
-                    if (mode == 3) pair_loop<3>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
-                    else pair_loop<2>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, m);
+                    int seg = n;                     // sources per flagged segment
+                    if (n <= kShortPass) {
+                        if (mode == 3) pair_loop<3, false>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits);
+                        else pair_loop<2, false>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits);
+                    } else {
+                        const int ntr = (n + 4 * kQuads - 1) / (4 * kQuads);
+                        const int sh = ntr > 32 ? 32 - __clz((ntr - 1) >> 5) : 0;     // (trips >> sh) < 32
+                        seg = (4 * kQuads) << sh;
+                        if (mode == 3) pair_loop<3, true>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, sh, bits);
+                        else pair_loop<2, true>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, sh, bits);
+                    }
 #pragma unroll
                     for (int j = 0; j < kS; ++j)
-                        if (m[j] < rc2)
-                            close_scan(K, S.xs, S.ys, S.zs, lo, lo + n, xim[j], yi[j], zi[j], rc2, fmax, S.hdr.g_lo, slot + j, ha, hb, dzc,
+                        if (bits[j])
+                            close_scan(K, S.xs, S.ys, S.zs, lo, lo + n, bits[j], seg, xim[j], yi[j], zi[j], rc2, fmax, S.hdr.g_lo, slot + j, ha, hb, dzc,
                                        &close_corr[0][tid_s + j]);
                 }
             };
