@@ -5,8 +5,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 does not import ``paper_2110_11392_b200``.  See ``nf_oracle.c`` for the definition it follows
 (PAPER.md:132 Eq. 3, :143, :218) and the list of pins.
 """
-from .nf_oracle import (accel, bin_particles, build, cell_lists, force_factor, max_threads,
+from .nf_oracle import (accel, accel_variant, bin_particles, build, cell_lists, force_factor, max_threads,
                         neighbors, pair_count, plummer_factor, lib_path)
 
-__all__ = ["accel", "bin_particles", "build", "cell_lists", "force_factor", "max_threads",
+__all__ = ["accel", "accel_variant", "bin_particles", "build", "cell_lists", "force_factor", "max_threads",
            "neighbors", "pair_count", "plummer_factor", "lib_path"]

@@ -248,3 +248,102 @@ int64_t nfo_accel(const float *pos, int64_t N, int cpd, int R, double eps_p, dou
     free(so); free(cell); free(off); free(offsets); free(order);
     return pairs;
 }
+
+/*
+ * Variants of the near-field sum the paper configures at build time (Fig. 19:
+ * "Near-force softening technique", "Compute FOF-scale density"), same loop nest and cell-pair
+ * definition as nfo_accel:
+ *   law = 0  spline softening, Eq. 3, eps_s = 2.16 eps_p
+ *   law = 1  Plummer softening, Eq. 2: F = r / (r^2 + eps_p^2)^(3/2)
+ *   dens_b > 0 and dens != NULL: the FoF-scale density estimate of sec. 3.4.4,
+ *       "an apodized top-hat density estimate 1 - r^2/b^2 (for r < b), which is computed as
+ *       b^2 - r^2 on the GPU":   dens_p = sum over sources q != p of the same (2R+1)^3 cells
+ *       with r < b of (b^2 - r^2), r = |d| the same separation the force uses.
+ *       Readings (D1-D3): the particle itself is not counted (q != p, as in the force
+ *       loop); a distinct particle at r = 0 counts b^2; the sum is left unnormalised in
+ *       (length unit)^2, as the paper's kernel leaves it.
+ * acc may be NULL (density only).  Returns pairs visited, or -1.
+ */
+int64_t nfo_accel_variant(const float *pos, int64_t N, int cpd, int R, double eps_p, double box, double gm, int law, double dens_b,
+                          const int32_t *sink_cells, int64_t n_sink_cells, double *acc, double *dens, int nthreads) {
+    if (N < 0 || R < 1 || cpd < 2 * R + 1 || !(eps_p > 0) || !(box > 0) || law < 0 || law > 1 || dens_b < 0) return -1;
+    const int64_t ncell = (int64_t)cpd * cpd * cpd;
+    const double cellsz = box / (double)cpd;
+    const double eps_s = NFO_SPLINE_PER_PLUMMER * eps_p;
+    const double b2 = dens_b * dens_b;
+    const int nn = (2 * R + 1) * (2 * R + 1) * (2 * R + 1);
+    int32_t *cell = (int32_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int32_t));
+    double *off = (double *)malloc((size_t)(N > 0 ? N : 1) * 3 * sizeof(double));
+    int64_t *offsets = (int64_t *)malloc((size_t)(ncell + 1) * sizeof(int64_t));
+    int64_t *order = (int64_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int64_t));
+    double *so = (double *)malloc((size_t)(N > 0 ? N : 1) * 3 * sizeof(double));
+    if (!cell || !off || !offsets || !order || !so || nfo_bin(pos, N, cpd, box, cell, off) != 0) {
+        free(cell); free(off); free(offsets); free(order); free(so);
+        return -1;
+    }
+    nfo_cell_lists(cell, N, ncell, offsets, order);
+    for (int64_t s = 0; s < N; ++s) {
+        int64_t i = order[s];
+        so[3 * s + 0] = off[3 * i + 0]; so[3 * s + 1] = off[3 * i + 1]; so[3 * s + 2] = off[3 * i + 2];
+    }
+    const int64_t nwork = sink_cells ? n_sink_cells : ncell;
+    int64_t pairs = 0;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel
+    {
+        int32_t *ids = (int32_t *)malloc((size_t)nn * sizeof(int32_t));
+        int8_t *img = (int8_t *)malloc((size_t)nn * 3);
+#pragma omp for schedule(dynamic, 1) reduction(+ : pairs)
+        for (int64_t w = 0; w < nwork; ++w) {
+            const int C = sink_cells ? sink_cells[w] : (int)w;
+            const int64_t p0 = offsets[C], p1 = offsets[C + 1];
+            if (p0 == p1) continue;
+            nfo_neighbors(cpd, R, C, ids, img);
+            for (int64_t p = p0; p < p1; ++p) {
+                double ax = 0.0, ay = 0.0, az = 0.0, wd = 0.0;
+                const double px = so[3 * p], py = so[3 * p + 1], pz = so[3 * p + 2];
+                int n = 0;
+                for (int a = -R; a <= R; ++a)
+                    for (int b = -R; b <= R; ++b)
+                        for (int c = -R; c <= R; ++c, ++n) {
+                            const int S = ids[n];
+                            const double sx = a * cellsz, sy = b * cellsz, sz = c * cellsz;
+                            const int64_t q0 = offsets[S], q1 = offsets[S + 1];
+                            for (int64_t q = q0; q < q1; ++q) {
+                                if (q == p) continue;
+                                const double dx = (so[3 * q] - px) + sx;
+                                const double dy = (so[3 * q + 1] - py) + sy;
+                                const double dz = (so[3 * q + 2] - pz) + sz;
+                                const double r2 = dx * dx + dy * dy + dz * dz;
+                                ++pairs;
+                                if (r2 < b2) wd += b2 - r2;
+                                if (r2 == 0.0) continue;                 /* F(0) = 0 for both laws */
+                                double f;
+                                if (law == 1) {
+                                    const double s2 = r2 + eps_p * eps_p;    /* Eq. 2 */
+                                    f = 1.0 / (s2 * sqrt(s2));
+                                } else {
+                                    const double r = sqrt(r2);
+                                    if (r < eps_s) {
+                                        const double u = r / eps_s;          /* Eq. 3 */
+                                        f = (10.0 - 15.0 * u + 6.0 * u * u) / (eps_s * eps_s * eps_s);
+                                    } else {
+                                        f = 1.0 / (r2 * r);
+                                    }
+                                }
+                                ax += gm * f * dx; ay += gm * f * dy; az += gm * f * dz;
+                            }
+                        }
+                const int64_t i = order[p];
+                if (acc) { acc[3 * i] = ax; acc[3 * i + 1] = ay; acc[3 * i + 2] = az; }
+                if (dens) dens[i] = wd;
+            }
+        }
+        free(ids);
+        free(img);
+    }
+    free(so); free(cell); free(off); free(offsets); free(order);
+    return pairs;
+}

@@ -70,6 +70,8 @@ def _load():
         L.nfo_pair_count.argtypes = [vp, i32, i32]
         L.nfo_accel.restype = i64
         L.nfo_accel.argtypes = [vp, i64, i32, i32, dbl, dbl, dbl, vp, i64, vp, i32]
+        L.nfo_accel_variant.restype = i64
+        L.nfo_accel_variant.argtypes = [vp, i64, i32, i32, dbl, dbl, dbl, i32, dbl, vp, i64, vp, vp, i32]
         _lib = L
     return _lib
 
@@ -152,3 +154,28 @@ def accel(pos, cpd: int, R: int, eps_p: float, box: float = 1.0, gm: float | Non
     if pairs < 0:
         raise ValueError("nfo_accel: bad arguments or non-finite position")
     return acc, int(pairs)
+
+
+def accel_variant(pos, cpd: int, R: int, eps_p: float, box: float = 1.0, gm: float | None = None,
+                  law: str = "spline", density_b: float = 0.0, sink_cells=None, nthreads: int = 0):
+    """The build-time variants of the paper's kernel, by the definition:
+    ``law`` = "spline" (Eq. 3) or "plummer" (Eq. 2); ``density_b`` > 0 adds the
+    FoF-scale density estimate sum_{q != p, r < b} (b^2 - r^2).
+    -> (acc[N,3] float64, dens[N] float64 or None, pairs visited)."""
+    p = _f32pos(pos)
+    N = p.shape[0]
+    if gm is None:
+        gm = 1.0 / max(N, 1)
+    acc = np.zeros((N, 3), dtype=np.float64)
+    dens = np.zeros(N, dtype=np.float64) if density_b > 0 else None
+    if sink_cells is None:
+        sc_ptr, nsc = None, 0
+    else:
+        sc = np.ascontiguousarray(sink_cells, dtype=np.int32)
+        sc_ptr, nsc = sc.ctypes.data, sc.shape[0]
+    pairs = _load().nfo_accel_variant(p.ctypes.data, N, cpd, R, float(eps_p), float(box), float(gm),
+                                      {"spline": 0, "plummer": 1}[law], float(density_b), sc_ptr, nsc,
+                                      acc.ctypes.data, dens.ctypes.data if dens is not None else None, int(nthreads))
+    if pairs < 0:
+        raise ValueError("nfo_accel_variant: bad arguments or non-finite position")
+    return acc, dens, int(pairs)
