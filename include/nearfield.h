@@ -49,6 +49,8 @@ typedef enum {
 } nf_status;
 
 #define NF_MAX_R 4          /* compiled maximum near-field radius */
+#define NF_SOFT_SPLINE 0    /* Eq. 3, the paper's "single_spline" (Fig. 19) */
+#define NF_SOFT_PLUMMER 1   /* Eq. 2 */
 #define NF_N_STAGES 8       /* entries of nf_stage_ms */
 
 /*
@@ -85,6 +87,33 @@ nf_status nf_set_gm(nf_ctx *ctx, double gm);
  * result is unspecified, and the next nf_sync returns NF_EPOS.
  */
 nf_status nf_accel(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc, void *cuda_stream);
+
+/*
+ * nf_set_softening -- the "near-force softening technique" the paper chooses at build time
+ * (PAPER.md:620): NF_SOFT_SPLINE (default; Eq. 3 with eps_s = 2.16 eps_plummer) or
+ * NF_SOFT_PLUMMER (Eq. 2, F = r/(r^2 + eps_plummer^2)^(3/2)).  Takes effect at the
+ * next nf_accel / nf_accel4.  NF_EINVAL: ctx NULL or an unknown law.
+ */
+nf_status nf_set_softening(nf_ctx *ctx, int law);
+
+/*
+ * nf_set_density_radius -- radius b (length units of box) of the FoF-scale density estimate
+ * of sec. 3.4.4 ("Compute FOF-scale density"), used by nf_accel4.
+ * b = 0 (default) switches it off.  NF_EINVAL: ctx NULL, b < 0 or not finite.
+ */
+nf_status nf_set_density_radius(nf_ctx *ctx, double b);
+
+/*
+ * nf_accel4 -- nf_accel with the accelerations "promoted to 4-vectors":
+ *   d_acc4 [out] device, N*4 floats (ax, ay, az, w) in INPUT order, where
+ *       w_i = sum over the sources j != i of the same (2R+1)^3 cells with r_ij < b of (b^2 - r_ij^2),
+ *   the paper's apodised top-hat estimate "computed as b^2 - r^2 on the GPU", unnormalised, in
+ *   (length unit)^2; the particle itself is not counted, a distinct particle at r = 0 counts b^2.
+ *   With b = 0 the 4th component is not written.
+ * Same kernels as nf_accel (the density rides in the near-cell form of the pair loop); same
+ * arguments, ordering and errors.
+ */
+nf_status nf_accel4(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc4, void *cuda_stream);
 
 /*
  * nf_accel_host -- the same through HOST buffers: copies h_pos to the device, runs

@@ -21,7 +21,8 @@ STAGE_NAMES = ["A1_key_hist", "A2_scan", "A3_scatter_rank_gather", "A4_scheduler
 # every symbol include/nearfield.h declares
 SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", "nf_sync",
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
-           "nf_interaction_count", "nf_probe_pipes", "nf_debug_read", "nf_launch_count", "nf_close_radius"]
+           "nf_interaction_count", "nf_probe_pipes", "nf_debug_read", "nf_launch_count", "nf_close_radius",
+           "nf_set_softening", "nf_set_density_radius", "nf_accel4"]
 
 
 class NearFieldError(RuntimeError):
@@ -50,6 +51,12 @@ def load_library() -> ctypes.CDLL:
     L.nf_set_gm.argtypes = [vp, dbl]
     L.nf_accel.restype = i32
     L.nf_accel.argtypes = [vp, vp, i64, vp, vp]
+    L.nf_accel4.restype = i32
+    L.nf_accel4.argtypes = [vp, vp, i64, vp, vp]
+    L.nf_set_softening.restype = i32
+    L.nf_set_softening.argtypes = [vp, i32]
+    L.nf_set_density_radius.restype = i32
+    L.nf_set_density_radius.argtypes = [vp, dbl]
     L.nf_accel_host.restype = i32
     L.nf_accel_host.argtypes = [vp, vp, i64, vp]
     L.nf_sync.restype = i32
@@ -147,6 +154,29 @@ class NearField:
         self._check(_L.nf_accel(self._h, pos.data_ptr() if N else None, N, acc.data_ptr() if N else None,
                                 ctypes.c_void_p(st.cuda_stream)))
         return acc
+
+    def set_softening(self, law: str):
+        """"spline" (Eq. 3, default) or "plummer" (Eq. 2) -- nf_set_softening"""
+        self._check(_L.nf_set_softening(self._h, {"spline": 0, "plummer": 1}[law]))
+
+    def set_density_radius(self, b: float):
+        self._check(_L.nf_set_density_radius(self._h, float(b)))
+
+    def accel4(self, pos, acc4=None, stream=None):
+        """nf_accel4: -> [N,4] (ax, ay, az, density estimate of PAPER.md:256)."""
+        import torch
+        if not (pos.is_cuda and pos.dtype == torch.float32 and pos.is_contiguous() and pos.dim() == 2 and pos.shape[1] == 3):
+            raise ValueError("pos must be a contiguous CUDA float32 tensor of shape [N,3]")
+        N = pos.shape[0]
+        if acc4 is None:
+            acc4 = torch.zeros((N, 4), dtype=torch.float32, device=pos.device)
+        elif not (acc4.is_cuda and acc4.dtype == torch.float32 and acc4.is_contiguous() and tuple(acc4.shape) == (N, 4)):
+            raise ValueError("acc4 must be a contiguous CUDA float32 tensor of shape [N,4]")
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        self._N = N
+        self._check(_L.nf_accel4(self._h, pos.data_ptr() if N else None, N, acc4.data_ptr() if N else None,
+                                 ctypes.c_void_p(st.cuda_stream)))
+        return acc4
 
     def accel_ptr(self, d_pos: int, N: int, d_acc: int, cuda_stream: int = 0):
         """raw-pointer form of nf_accel (used by tests of the error paths)."""

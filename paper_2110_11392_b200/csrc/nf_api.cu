@@ -146,7 +146,21 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
     return NF_OK;
 }
 
-extern "C" nf_status nf_accel(nf_ctx *c, const float *d_pos, int64_t N, float *d_acc, void *cuda_stream) {
+extern "C" nf_status nf_set_softening(nf_ctx *c, int law) {
+    if (!c) return NF_EINVAL;
+    if (law != NF_SOFT_SPLINE && law != NF_SOFT_PLUMMER) { snprintf(c->err, sizeof c->err, "nf_set_softening: unknown law %d", law); return NF_EINVAL; }
+    c->law = law;
+    return NF_OK;
+}
+
+extern "C" nf_status nf_set_density_radius(nf_ctx *c, double b) {
+    if (!c) return NF_EINVAL;
+    if (!(b >= 0) || !isfinite(b)) { snprintf(c->err, sizeof c->err, "nf_set_density_radius: need a finite b >= 0"); return NF_EINVAL; }
+    c->dens_b = b;
+    return NF_OK;
+}
+
+static nf_status accel_any(nf_ctx *c, const float *d_pos, int64_t N, float *d_acc, int ostride, void *cuda_stream) {
     if (!c) return NF_EINVAL;
     c->err[0] = 0;
     if (N < 0 || (N > 0 && (!d_pos || !d_acc)) || (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
@@ -168,10 +182,18 @@ extern "C" nf_status nf_accel(nf_ctx *c, const float *d_pos, int64_t N, float *d
     const double gm = c->gm > 0 ? c->gm : 1.0 / (double)N;
     const double cellsz = c->box / (double)c->cpd;
     const float kfac = (float)(gm / (cellsz * cellsz));
-    rc = nf_run_interact(c, d_pos, N, d_acc, kfac, st);
+    rc = nf_run_interact(c, d_pos, N, d_acc, ostride, kfac, st);
     if (rc != NF_OK) return rc;
     if (c->opt_stage_timing) { cudaEventRecord(c->ev[5], st); cudaEventRecord(c->ev[7], st); }
     return NF_OK;
+}
+
+extern "C" nf_status nf_accel(nf_ctx *c, const float *d_pos, int64_t N, float *d_acc, void *cuda_stream) {
+    return accel_any(c, d_pos, N, d_acc, 3, cuda_stream);
+}
+
+extern "C" nf_status nf_accel4(nf_ctx *c, const float *d_pos, int64_t N, float *d_acc4, void *cuda_stream) {
+    return accel_any(c, d_pos, N, d_acc4, 4, cuda_stream);
 }
 
 extern "C" nf_status nf_sync(nf_ctx *c) {

@@ -68,6 +68,8 @@ struct NfBlockDesc {     // one sink work item: <= NF_BS consecutive padded slot
 struct nf_ctx {
     int device, cpd, R, sm_count;
     double eps_p, box, gm;
+    int law;                     // NF_SOFT_SPLINE | NF_SOFT_PLUMMER
+    double dens_b;               // FoF-scale density radius (length units); 0 = off
     int64_t ncell, ncol;
     NfParams prm;
     // options
@@ -110,7 +112,7 @@ struct nf_ctx {
 // stages implemented in the other translation units
 nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st);
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st);
-nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc, float kfac, cudaStream_t st);
+nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st);
 nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st);
 nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_interact_setup(nf_ctx *ctx);

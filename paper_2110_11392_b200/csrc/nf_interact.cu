@@ -134,7 +134,8 @@ __global__ void __launch_bounds__(256) k_density(int ncell, const uint32_t *__re
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
     if ((threadIdx.x & 31) == 0 && v) atomicAdd(sum2, v);
 }
-__global__ void k_choose_rc(const unsigned long long *__restrict__ sum2, double N, double eps_cells, float rc_override, float *__restrict__ dyn) {
+__global__ void k_choose_rc(const unsigned long long *__restrict__ sum2, double N, double eps_cells, double soft2, float rc_override,
+                            float *__restrict__ dyn) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     double rc;
     if (rc_override >= 0.f) {
@@ -154,7 +155,10 @@ __global__ void k_choose_rc(const unsigned long long *__restrict__ sum2, double 
     }
     dyn[0] = (float)(rc * rc);
     dyn[1] = (float)rc;
-    dyn[2] = rc > 0.0 ? (float)(1.0 / (rc * rc * rc)) : 0.f;   // clamp of the float32 r^-3 in near cells
+    // soft2 = eps_p^2 (cell units) for Plummer softening (the loop's r^2 carries it), 0 for the spline
+    const double rs2 = rc * rc + soft2;
+    dyn[2] = rc > 0.0 ? (float)(1.0 / (rs2 * sqrt(rs2))) : 0.f;   // clamp of the float32 force factor in near cells
+    dyn[3] = (float)rs2;                                           // what the loop's r^2 (+ soft2) is compared with
 }
 
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st) {
@@ -162,7 +166,12 @@ nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st) {
     unsigned long long *sum2 = (unsigned long long *)(ctx->d_ctrl + 100);
     NF_CUDA_OK(ctx, cudaMemsetAsync(sum2, 0, 8, st));
     k_density<<<((int)ctx->ncell + 255) / 256, 256, 0, st>>>((int)ctx->ncell, ctx->d_counts, sum2); ctx->launches++;
-    k_choose_rc<<<1, 32, 0, st>>>(sum2, (double)N, ctx->prm.eps_cells, ctx->opt_rc, (float *)(ctx->d_ctrl + 96)); ctx->launches++;
+    {
+        const double ep = ctx->eps_p * ctx->prm.scale;       // eps_p in cell units
+        const bool plummer = ctx->law == NF_SOFT_PLUMMER;
+        k_choose_rc<<<1, 32, 0, st>>>(sum2, (double)N, plummer ? ep : ctx->prm.eps_cells, plummer ? ep * ep : 0.0, ctx->opt_rc,
+                                      (float *)(ctx->d_ctrl + 96)); ctx->launches++;
+    }
     k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk); ctx->launches++;
     nf_status rc = nf_scan_u32(ctx, ctx->d_col_nblk, (uint32_t)ncol, ctx->d_col_base, st);
     if (rc != NF_OK) return rc;
@@ -212,6 +221,11 @@ struct InteractArgs {
     const float *dyn;        // [0] rc^2 (cell units^2; 0 = no close-pair radius, use the min form)  [1] rc  [2] rc^-3
     float *acc;
     float kfac;
+    float addend;            // addend of r^2: NF_TAU (spline) or eps_p^2 in cell units (Plummer, Eq. 2)
+    float b2;                // density radius^2 (cell units) + addend; DENS only
+    float wfac;              // cell^2: density sum to length units
+    int ostride;             // floats per output particle: 3, or 4 with the density estimate in the 4th
+    int near_cheb;           // cells within this Chebyshev distance run the near-cell form
     NfParams prm;
 };
 
@@ -232,6 +246,9 @@ struct CloseArgs {
     const uint32_t *perm_pad;  // padded slot -> input index
     double scale;              // cpd / box
     double eps;                // eps_s in cell units
+    double soft2;              // eps_p^2 in cell units (Plummer) or 0
+    float addend;              // the loop's r^2 addend
+    int law;
 };
 __device__ __forceinline__ double exact_offset(float x, double scale) {
     const double t = (double)x * scale;
@@ -253,7 +270,7 @@ __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, con
     const int s1 = (s0 + seg < hi) ? s0 + seg : hi;
     for (int s = s0; s < s1; ++s) {
         const float dxf = __fadd_rn(xs[s], -xim), dyf = __fadd_rn(ys[s], -yi), dzf = __fadd_rn(zs[s], -zi);
-        float r2f = __fmaf_rn(dxf, dxf, NF_TAU);
+        float r2f = __fmaf_rn(dxf, dxf, K.addend);
         r2f = __fmaf_rn(dyf, dyf, r2f);
         r2f = __fmaf_rn(dzf, dzf, r2f);
         if (!(r2f < rc2)) continue;
@@ -269,7 +286,10 @@ __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, con
         if (r2 == 0.0) continue;                          // coincident particles: F(0) = 0
         const double r = sqrt(r2);
         double f;
-        if (r < K.eps) {
+        if (K.law == NF_SOFT_PLUMMER) {
+            const double s2 = r2 + K.soft2;               // Eq. 2
+            f = 1.0 / (s2 * sqrt(s2));
+        } else if (r < K.eps) {
             const double u = r / K.eps;
             f = (10.0 - 15.0 * u + 6.0 * u * u) / (K.eps * K.eps * K.eps);
         } else {
@@ -297,12 +317,14 @@ __device__ __forceinline__ float fmin3(float a, float b, float c) {
 constexpr int kS = NF_SINKS;
 constexpr int kQuads = NF_QUADS_PER_TRIP;
 constexpr int kShortPass = 96;                       // passes up to this many sources flag close pairs per pass, longer ones per trip
-template <int MODE, bool TRIPBITS>
+template <int MODE, bool TRIPBITS, int LAW, bool DENS>
 __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const float *__restrict__ ys, const float *__restrict__ zs, int lo, int n,
                                           const float (&xim)[kS], const float (&yi)[kS], const float (&zi)[kS], float2 (&ax)[kS],
                                           float2 (&ay)[kS], float2 (&az)[kS], const float2 c0, const float2 c1, const float2 c2,
-                                          const float fmax, const float rc2, const int sh, uint32_t (&bits)[kS]) {
-    const float2 tau = make_float2(NF_TAU, NF_TAU);
+                                          const float fmax, const float rc2, const int sh, uint32_t (&bits)[kS], const float addend,
+                                          const float b2, float2 (&aw)[kS]) {
+    const float2 tau = (LAW == 0) ? make_float2(NF_TAU, NF_TAU) : make_float2(addend, addend);   // an immediate for the spline
+    const float2 b2v = make_float2(b2, b2);
     float2 nx[kS], ny[kS], nz[kS];
 #pragma unroll
     for (int j = 0; j < kS; ++j) { nx[j] = make_float2(-xim[j], -xim[j]); ny[j] = make_float2(-yi[j], -yi[j]); nz[j] = make_float2(-zi[j], -zi[j]); }
@@ -315,7 +337,7 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
         const float2 ri = make_float2(mufu_rsq(r2.x), mufu_rsq(r2.y));
         const float2 ri2 = __fmul2_rn(ri, ri);
         float2 f = __fmul2_rn(ri2, ri);                    // r^-3
-        if (MODE == 1) {
+        if (MODE == 1 && LAW == 0) {
             const float2 r = __fmul2_rn(r2, ri);           // r
             float2 h = __ffma2_rn(r, c2, c1);
             h = __ffma2_rn(r, h, c0);                      // (10 - 15u + 6u^2)/eps^3
@@ -325,8 +347,12 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
         if (MODE >= 2) {
             f.x = fminf(f.x, fmax);
             f.y = fminf(f.y, fmax);
-            if (MODE == 2) m[j] = fmin3(m[j], r2.x, r2.y);
+            if (MODE == 2 || LAW != 0) m[j] = fmin3(m[j], r2.x, r2.y);   // Plummer: the self pair is flagged and dropped by close_scan
             else m[j] = fmin3(m[j], r2.x > 2.f * NF_TAU ? r2.x : NF_BIG, r2.y > 2.f * NF_TAU ? r2.y : NF_BIG);
+        }
+        if (DENS && MODE >= 1) {                           // b^2 - r^2 for r < b; the self pair's b^2 is taken off at the end
+            const float2 t = __fadd2_rn(b2v, make_float2(-r2.x, -r2.y));
+            aw[j] = __fadd2_rn(aw[j], make_float2(fmaxf(t.x, 0.f), fmaxf(t.y, 0.f)));
         }
         ax[j] = __ffma2_rn(f, dx, ax[j]);
         ay[j] = __ffma2_rn(f, dy, ay[j]);
@@ -397,13 +423,15 @@ __device__ __forceinline__ void fold(float &tot, float &comp, float v, int kahan
 // FLAG = the regime k_choose_rc picked on the device: true = a close-pair radius is in use
 // (near cells: clamp + close_scan), false = Eq. 3 as a min in near cells.  Both instantiations
 // are launched; the one whose regime is not in force returns at once (no host round trip).
-template <bool FLAG>
+// LAW: NF_SOFT_SPLINE (Eq. 3) or NF_SOFT_PLUMMER (Eq. 2).  DENS: also accumulate the FoF-scale density
+// estimate in the near cells and store it as the 4th output component.
+template <bool FLAG, int LAW, bool DENS>
 __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(const InteractArgs A) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Stage *stages = reinterpret_cast<Stage *>(smem_raw);
     __shared__ uint64_t full_bar[NF_NSTAGE], empty_bar[NF_NSTAGE];
     __shared__ double close_corr[3][NF_BS];
-    __shared__ float tot[6][NF_BS];      // per sink: running sums x, y, z and their Kahan compensations
+    __shared__ float tot[DENS ? 7 : 6][NF_BS];   // per sink: running sums x, y, z, their Kahan compensations, density sum
     if ((A.dyn[0] > 0.f) != FLAG) return;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -506,11 +534,12 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
     // Thread t of warp w holds the kS sinks at slots s0 + (32 w + t) kS + j of the block (adjacent
     // slots: cells are padded to 4 slots and blocks start on multiples of 4, so they share a cell).
     const float2 c0 = make_float2(A.prm.c0, A.prm.c0), c1 = make_float2(A.prm.c1, A.prm.c1), c2 = make_float2(A.prm.c2, A.prm.c2);
-    const int near_cheb = A.prm.near_cheb, kahan = A.prm.kahan;
-    const float rc2 = A.dyn[0];
+    const int near_cheb = A.near_cheb, kahan = A.prm.kahan;
+    const float rc2 = A.dyn[3];
     const float fmax = A.dyn[2];
     CloseArgs K;
     K.pos = A.pos; K.perm_pad = A.perm_pad; K.scale = A.prm.scale; K.eps = A.prm.eps_cells;
+    K.law = LAW; K.addend = A.addend; K.soft2 = (LAW == NF_SOFT_PLUMMER) ? (double)A.addend : 0.0;
     const int tid_s = (int)threadIdx.x * kS;           // this thread's first column of close_corr / tot
     float px[kS], py[kS], pz[kS];
 #pragma unroll
@@ -547,7 +576,7 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
 #pragma unroll
             for (int j = 0; j < kS; ++j) {
 #pragma unroll
-                for (int q = 0; q < 6; ++q) tot[q][tid_s + j] = 0.f;
+                for (int q = 0; q < (DENS ? 7 : 6); ++q) tot[q][tid_s + j] = 0.f;
 #pragma unroll
                 for (int q = 0; q < 3; ++q) close_corr[q][tid_s + j] = 0.0;
             }
@@ -565,21 +594,27 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
             int nz0 = 1 << 30, nz1 = -(1 << 30), hz0 = 1 << 30, hz1 = -(1 << 30);
             if (abs(ha) <= near_cheb && abs(hb) <= near_cheb) { nz0 = z1 - near_cheb; nz1 = z2 + near_cheb; }
             if (ha == 0 && hb == 0) { hz0 = z1; hz1 = z2; }
-            auto mode_of = [&](int zu) { return (zu < nz0 || zu > nz1) ? 0 : (!FLAG ? 1 : ((zu >= hz0 && zu <= hz1) ? 3 : 2)); };
+            // far cells 0; near cells: 1 without a close-pair radius (Eq. 3 as a min; Plummer: density only), 2/3 with one
+            auto mode_of = [&](int zu) { return (zu < nz0 || zu > nz1) ? 0 : (!FLAG ? ((LAW == 0 || DENS) ? 1 : 0) : ((zu >= hz0 && zu <= hz1) ? 3 : 2)); };
             const int *tab = reinterpret_cast<const int *>(S.tab) - zu0;   // tab[zu] = first stage-local slot of source cell zu
-            float2 ax[kS], ay[kS], az[kS];
+            float2 ax[kS], ay[kS], az[kS], aw[kS];
 #pragma unroll
-            for (int j = 0; j < kS; ++j) { ax[j] = make_float2(0.f, 0.f); ay[j] = ax[j]; az[j] = ax[j]; }
+            for (int j = 0; j < kS; ++j) { ax[j] = make_float2(0.f, 0.f); ay[j] = ax[j]; az[j] = ax[j]; aw[j] = ax[j]; }
 
             // One pass = sources [lo, lo + n) where a lane reads cell cA's part (from loA) if its
             // sink is within R cells of cA, else cell cB's part (from loB) if within R of cB, else
             // it is masked.  cB = cA + 2R+1, so the two lane groups are disjoint: the edge cells
             // of the warp's window, each needed by only part of the warp, are processed two at a
             // time and no lane idles.
-            auto pass = [&](int loA, int cA, int loB, int cB, int n, int mode) {
-                const bool useA = abs(zl - cA) <= R, useB = abs(zl - cB) <= R;
-                const int cell = useA ? cA : cB;
-                const int lo = useA ? loA : loB;
+            // One pass = sources [lo, lo + n) where a lane reads cell cA's part (from loA) if its
+            // sink is within R cells of cA, else cell cB's part (from loB) if within R of cB, else
+            // it is masked.  cB = cA + 2R+1, so the two lane groups are disjoint: the edge cells
+            // of the warp's window, each needed by only part of the warp, are processed two at a
+            // time and no lane idles.
+            auto pass = [&](const int ploA, const int pcA, const int ploB, const int pcB, const int n, const int mode) __attribute__((always_inline)) {
+                const bool useA = abs(zl - pcA) <= R, useB = abs(zl - pcB) <= R;
+                const int cell = useA ? pcA : pcB;
+                const int lo = useA ? ploA : ploB;
                 const int dzc = cell - zl;
                 float xim[kS], zi[kS];
                 uint32_t bits[kS];
@@ -589,19 +624,19 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
                     zi[j] = pz[j] - (float)dzc;
                     bits[j] = 0u;
                 }
-                if (mode == 0) pair_loop<0, false>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits);
-                else if (!FLAG) pair_loop<1, false>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits);
+                if (mode == 0) pair_loop<0, false, LAW, DENS>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits, A.addend, A.b2, aw);
+                else if (!FLAG) pair_loop<1, false, LAW, DENS>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits, A.addend, A.b2, aw);
                 else {
                     int seg = n;                     // sources per flagged segment
                     if (n <= kShortPass) {
-                        if (mode == 3) pair_loop<3, false>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits);
-                        else pair_loop<2, false>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits);
+                        if (mode == 3) pair_loop<3, false, LAW, DENS>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits, A.addend, A.b2, aw);
+                        else pair_loop<2, false, LAW, DENS>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits, A.addend, A.b2, aw);
                     } else {
                         const int ntr = (n + 4 * kQuads - 1) / (4 * kQuads);
                         const int sh = ntr > 32 ? 32 - __clz((ntr - 1) >> 5) : 0;     // (trips >> sh) < 32
                         seg = (4 * kQuads) << sh;
-                        if (mode == 3) pair_loop<3, true>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, sh, bits);
-                        else pair_loop<2, true>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, sh, bits);
+                        if (mode == 3) pair_loop<3, true, LAW, DENS>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, sh, bits, A.addend, A.b2, aw);
+                        else pair_loop<2, true, LAW, DENS>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, sh, bits, A.addend, A.b2, aw);
                     }
 #pragma unroll
                     for (int j = 0; j < kS; ++j)
@@ -617,12 +652,15 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
                     const int cB = cA + W;
                     const int a0 = tab[cA], a1 = tab[cA + 1];
                     int b0 = 0, b1 = 0;
-                    int mA = mode_of(cA), mB = 0;
+                    const int mA = mode_of(cA);
+                    int mB = 0;
                     if (cB <= cz1) { b0 = tab[cB]; b1 = tab[cB + 1]; mB = mode_of(cB); }
                     const int nA = a1 - a0, nB = b1 - b0;
                     const int ncm = nA < nB ? nA : nB;
+                    // the common length of the two cells, both lane groups at once; then the rest of
+                    // the longer cell, its own lanes only
                     if (ncm > 0) pass(a0, cA, b0, cB, ncm, mA > mB ? mA : mB);
-                    if (nA > ncm) pass(a0 + ncm, cA, 0, -(1 << 28), nA - ncm, mA);          // rest of the longer cell: its own lanes only
+                    if (nA > ncm) pass(a0 + ncm, cA, 0, -(1 << 28), nA - ncm, mA);
                     else if (nB > ncm) pass(b0 + ncm, cB, 0, -(1 << 28), nB - ncm, mB);
                 }
             }
@@ -635,6 +673,7 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
                     fold(t, c, v[q], kahan);
                     tot[q][tid_s + j] = t; tot[q + 3][tid_s + j] = c;
                 }
+                if (DENS) tot[DENS ? 6 : 0][tid_s + j] += aw[j].x + aw[j].y;
             }
         }
         if (flags & NF_F_LAST) {
@@ -643,10 +682,12 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
                 for (int j = 0; j < kS; ++j) {
                     const uint32_t dst = A.perm_pad[slot + j];
                     if (dst != 0xffffffffu) {
-                        float *o = A.acc + 3ull * dst;
+                        float *o = A.acc + (size_t)A.ostride * dst;
                         o[0] = (float)((double)A.kfac * ((double)tot[0][tid_s + j] + close_corr[0][tid_s + j]));
                         o[1] = (float)((double)A.kfac * ((double)tot[1][tid_s + j] + close_corr[1][tid_s + j]));
                         o[2] = (float)((double)A.kfac * ((double)tot[2][tid_s + j] + close_corr[2][tid_s + j]));
+                        // density: the sink met itself exactly once (r = 0 -> b^2); take that off (reading D1)
+                        if (DENS) o[3] = (float)((double)A.wfac * ((double)tot[DENS ? 6 : 0][tid_s + j] - ((double)A.b2 - (double)A.addend)));
                     }
                 }
             }
@@ -659,31 +700,61 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
 
 static int g_interact_blocks_per_sm = 0;
 
+typedef void (*InteractKernel)(const InteractArgs);
+// [law][dens][flag]
+static InteractKernel interact_kernel(int law, int dens, int flag) {
+    static const InteractKernel tab[2][2][2] = {
+        {{k_interact<false, NF_SOFT_SPLINE, false>, k_interact<true, NF_SOFT_SPLINE, false>},
+         {k_interact<false, NF_SOFT_SPLINE, true>, k_interact<true, NF_SOFT_SPLINE, true>}},
+        {{k_interact<false, NF_SOFT_PLUMMER, false>, k_interact<true, NF_SOFT_PLUMMER, false>},
+         {k_interact<false, NF_SOFT_PLUMMER, true>, k_interact<true, NF_SOFT_PLUMMER, true>}}};
+    return tab[law][dens][flag];
+}
+
 nf_status nf_interact_setup(nf_ctx *ctx) {
     const size_t smem = sizeof(Stage) * NF_NSTAGE;
-    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_interact<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_interact<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int nb = 0;
-    NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_interact<true>, (NF_NW + 1) * 32, smem));
-    int nb2 = 0;
-    NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb2, k_interact<false>, (NF_NW + 1) * 32, smem));
-    if (nb2 < nb) nb = nb2;
+    int nb = 1 << 30;
+    for (int law = 0; law < 2; ++law)
+        for (int dens = 0; dens < 2; ++dens)
+            for (int flag = 0; flag < 2; ++flag) {
+                InteractKernel k = interact_kernel(law, dens, flag);
+                NF_CUDA_OK(ctx, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                int n1 = 0;
+                NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n1, k, (NF_NW + 1) * 32, smem));
+                if (n1 < nb) nb = n1;
+            }
     if (nb < 1) { snprintf(ctx->err, sizeof(ctx->err), "interaction kernel does not fit on an SM"); return NF_ECUDA; }
     g_interact_blocks_per_sm = nb;
     return NF_OK;
 }
 
-nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc, float kfac, cudaStream_t st) {
+// d_out: N x ostride floats (ostride 3: accelerations; 4: accelerations + density estimate)
+nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st) {
     InteractArgs A;
     A.pos = d_pos;
     A.sx = ctx->d_sorted; A.sy = ctx->d_sorted + ctx->capPad; A.sz = ctx->d_sorted + 2ull * ctx->capPad;
     A.skey = (const uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
     A.poff = ctx->d_poff; A.perm_pad = ctx->d_perm_pad; A.order = ctx->d_blk_order; A.blk = ctx->d_blk;
-    A.ctrl = ctx->d_ctrl; A.dyn = (const float *)(ctx->d_ctrl + 96); A.acc = d_acc; A.kfac = kfac; A.prm = ctx->prm;
+    A.ctrl = ctx->d_ctrl; A.dyn = (const float *)(ctx->d_ctrl + 96); A.acc = d_out; A.kfac = kfac; A.prm = ctx->prm;
     A.prm.kahan = ctx->opt_kahan;
+    A.ostride = ostride;
+    const int law = ctx->law == NF_SOFT_PLUMMER ? 1 : 0;
+    const int dens = (ostride == 4 && ctx->dens_b > 0.0) ? 1 : 0;
+    const double ep = ctx->eps_p * ctx->prm.scale;            // eps_p in cell units
+    A.addend = law ? (float)(ep * ep) : NF_TAU;
+    const double bc = ctx->dens_b * ctx->prm.scale;           // density radius in cell units
+    A.b2 = (float)(bc * bc) + A.addend;
+    const double cellsz = ctx->box / (double)ctx->cpd;
+    A.wfac = (float)(cellsz * cellsz);
+    // near cells: may hold r < eps_s (spline), or r < b (density)
+    int nc = law ? 1 : ctx->prm.near_cheb;
+    if (dens) { const int nb = (int)ceil(bc); if (nb > nc) nc = nb; }
+    if (nc > ctx->R) nc = ctx->R;
+    A.near_cheb = nc;
     const int grid = ctx->sm_count * g_interact_blocks_per_sm;
-    k_interact<true><<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
-    k_interact<false><<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
+    for (int flag = 1; flag >= 0; --flag) {     // the instantiation whose regime is not in force returns at once
+        interact_kernel(law, dens, flag)<<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
+    }
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }
