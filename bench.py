@@ -174,6 +174,52 @@ def time_oracle(cfg, pos, target_s: float, steps: int = 1, warmup: int = 0):
     return p3 * len(times) / tot, cores, sample, 1e3 * tot / len(times)
 
 
+def bench_slabs(args, cfg, workload, dist, rank, world, local_rank, barrier):
+    """N > 1, --parallel slabs: the same particle set on every rank (seed 0), each rank owns a
+    pair-balanced range of x slabs; a step = halo exchange (NCCL isend/irecv) + nf_accel on own +
+    ghost particles with only the own slabs as sinks.  value = all pairs / max-over-ranks time."""
+    import torch
+    from paper_2110_11392_b200 import slabs
+    from paper_2110_11392_b200 import workloads as W
+    pos_all = torch.from_numpy(W.make_positions(cfg)).cuda()
+    counts = torch.bincount(slabs.cell_index(pos_all, cfg.cpd, cfg.box), minlength=cfg.cpd ** 3)
+    bounds = slabs.balance_slabs(slabs.pairs_per_slab(counts, cfg.cpd, cfg.R), world)
+    own, _ = slabs.local_with_ghosts(pos_all, bounds, cfg.cpd, cfg.R, rank, cfg.box)
+    own = own.contiguous()
+    del pos_all, counts
+    snf = slabs.SlabNearField(cfg.cpd, cfg.R, cfg.eps_p, cfg.box, bounds)
+    snf.nf.set_gm(1.0 / cfg.N)
+    for _ in range(args.warmup):
+        acc = snf.accel(own)
+    torch.cuda.synchronize()
+    pairs_local = snf.interaction_count()
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    l0 = snf.nf.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        acc = snf.accel(own)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = snf.nf.launch_count() - l0
+    units, total_ms = aggregate_over_ranks(float(pairs_local) * args.steps, ev0.elapsed_time(ev1), dist)
+    ok = bool(torch.isfinite(acc[:: max(1, acc.shape[0] // 100003)]).all())
+    if rank == 0:
+        workload = dict(workload, parallelism=f"x-slab decomposition over {world} GPUs, R-slab halo exchange per step",
+                        slab_bounds=bounds)
+        print(json.dumps({"metric": METRIC, "value": units / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                          "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload,
+                          "sink_updates_per_s": cfg.N * args.steps / (total_ms * 1e-3), "pairs_per_step": units / args.steps,
+                          "clocks": clocks, "e2e": None, "gpu_launches": launches, "roofline": None, "cpu_baseline": None,
+                          "ghost_particles_rank0": snf.n_ghost, "result_finite": ok}))
+    dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -184,6 +230,9 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (weak scaling, default) or ONE particle set cut into x slabs "
+                         "with an R-slab halo exchange per step (strong scaling; paper_2110_11392_b200/slabs.py)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print(f"note: --warmup {args.warmup} < 3 breaks the timing rules", file=sys.stderr)
@@ -234,6 +283,8 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.parallel == "slabs" and world > 1:
+        return bench_slabs(args, base, workload, dist, rank, world, local_rank, barrier)
     pos = W.make_positions(cfg)
     nf = NearField(cfg.cpd, cfg.R, cfg.eps_p, cfg.box)
     nf.set_option("stage_timing", 1)

@@ -104,6 +104,19 @@ nf_status nf_set_softening(nf_ctx *ctx, int law);
 nf_status nf_set_density_radius(nf_ctx *ctx, double b);
 
 /*
+ * nf_set_sink_slabs -- slab decomposition (PAPER.md:80 "1-D slab decomposition", :413): only
+ * particles whose x cell index lies in the periodic range [x0, x0 + nx) are SINKS of the
+ * following nf_accel / nf_accel4 calls; every particle passed in is still a source.  A rank
+ * that owns those slabs passes its own particles plus the ghost particles of the R slabs on
+ * either side (near-field radius, Table 1) and reads back its own particles'
+ * rows; rows of non-sink particles are left untouched.  nf_interaction_count then counts the
+ * pairs of the sink cells only, so the counts of a complete decomposition add up to the
+ * single-GPU count.  Default: x0 = 0, nx = cpd (everything).  NF_EINVAL: ctx NULL, x0 outside
+ * [0, cpd), nx outside [1, cpd].
+ */
+nf_status nf_set_sink_slabs(nf_ctx *ctx, int x0, int nx);
+
+/*
  * nf_accel4 -- nf_accel with the accelerations "promoted to 4-vectors":
  *   d_acc4 [out] device, N*4 floats (ax, ay, az, w) in INPUT order, where
  *       w_i = sum over the sources j != i of the same (2R+1)^3 cells with r_ij < b of (b^2 - r_ij^2),

@@ -22,7 +22,7 @@ STAGE_NAMES = ["A1_key_hist", "A2_scan", "A3_scatter_rank_gather", "A4_scheduler
 SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", "nf_sync",
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
            "nf_interaction_count", "nf_probe_pipes", "nf_debug_read", "nf_launch_count", "nf_close_radius",
-           "nf_set_softening", "nf_set_density_radius", "nf_accel4"]
+           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs"]
 
 
 class NearFieldError(RuntimeError):
@@ -55,6 +55,8 @@ def load_library() -> ctypes.CDLL:
     L.nf_accel4.argtypes = [vp, vp, i64, vp, vp]
     L.nf_set_softening.restype = i32
     L.nf_set_softening.argtypes = [vp, i32]
+    L.nf_set_sink_slabs.restype = i32
+    L.nf_set_sink_slabs.argtypes = [vp, i32, i32]
     L.nf_set_density_radius.restype = i32
     L.nf_set_density_radius.argtypes = [vp, dbl]
     L.nf_accel_host.restype = i32
@@ -158,6 +160,10 @@ class NearField:
     def set_softening(self, law: str):
         """"spline" (Eq. 3, default) or "plummer" (Eq. 2) -- nf_set_softening"""
         self._check(_L.nf_set_softening(self._h, {"spline": 0, "plummer": 1}[law]))
+
+    def set_sink_slabs(self, x0: int, nx: int):
+        """only particles in x slabs [x0, x0 + nx) (periodic) are sinks -- nf_set_sink_slabs"""
+        self._check(_L.nf_set_sink_slabs(self._h, int(x0), int(nx)))
 
     def set_density_radius(self, b: float):
         self._check(_L.nf_set_density_radius(self._h, float(b)))

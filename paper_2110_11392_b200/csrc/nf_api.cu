@@ -41,6 +41,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     c->device = dev; c->cpd = cpd; c->R = R; c->eps_p = eps_plummer; c->box = box; c->gm = 0.0;
     c->sm_count = prop.multiProcessorCount;
     c->ncell = (int64_t)cpd * cpd * cpd; c->ncol = (int64_t)cpd * cpd;
+    c->slab_x0 = 0; c->slab_nx = cpd;
     c->opt_kahan = 1; c->opt_heavy_first = 0; c->opt_stage_timing = 0; c->opt_rc = -1.f;
     NfParams &p = c->prm;
     p.cpd = cpd; p.R = R; p.ncell = (int)c->ncell; p.ncol = (int)c->ncol;
@@ -70,7 +71,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     TRY_ALLOC(c->d_col_nblk, (size_t)(c->ncol + 1) * 4);
     TRY_ALLOC(c->d_col_base, (size_t)(c->ncol + 1) * 4);
     TRY_ALLOC(c->d_ctrl, 128 * 4);
-    TRY_ALLOC(c->d_pairs, 8);
+    TRY_ALLOC(c->d_pairs, 16);
     TRY_ALLOC(c->d_nbr, (size_t)4 * 729 * 4);
 #undef TRY_ALLOC
     for (int i = 0; i < 8; ++i)
@@ -150,6 +151,16 @@ extern "C" nf_status nf_set_softening(nf_ctx *c, int law) {
     if (!c) return NF_EINVAL;
     if (law != NF_SOFT_SPLINE && law != NF_SOFT_PLUMMER) { snprintf(c->err, sizeof c->err, "nf_set_softening: unknown law %d", law); return NF_EINVAL; }
     c->law = law;
+    return NF_OK;
+}
+
+extern "C" nf_status nf_set_sink_slabs(nf_ctx *c, int x0, int nx) {
+    if (!c) return NF_EINVAL;
+    if (x0 < 0 || x0 >= c->cpd || nx < 1 || nx > c->cpd) {
+        snprintf(c->err, sizeof c->err, "nf_set_sink_slabs: need 0 <= x0 < cpd and 1 <= nx <= cpd (x0=%d nx=%d)", x0, nx);
+        return NF_EINVAL;
+    }
+    c->slab_x0 = x0; c->slab_nx = nx;
     return NF_OK;
 }
 
@@ -303,9 +314,9 @@ extern "C" nf_status nf_interaction_count(nf_ctx *c, int64_t *h_pairs) {
     NF_CUDA_OK(c, cudaStreamSynchronize(c->last_stream));
     nf_status rc = nf_run_paircount(c, c->own_stream);
     if (rc != NF_OK) return rc;
-    unsigned long long v = 0;
-    NF_CUDA_OK(c, cudaMemcpyAsync(&v, c->d_pairs, 8, cudaMemcpyDeviceToHost, c->own_stream));
+    unsigned long long v[2] = {0, 0};
+    NF_CUDA_OK(c, cudaMemcpyAsync(v, c->d_pairs, 16, cudaMemcpyDeviceToHost, c->own_stream));
     NF_CUDA_OK(c, cudaStreamSynchronize(c->own_stream));
-    *h_pairs = (int64_t)v - c->lastN;
+    *h_pairs = (int64_t)v[0] - (int64_t)v[1];
     return NF_OK;
 }

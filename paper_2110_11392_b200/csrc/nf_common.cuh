@@ -70,6 +70,7 @@ struct nf_ctx {
     double eps_p, box, gm;
     int law;                     // NF_SOFT_SPLINE | NF_SOFT_PLUMMER
     double dens_b;               // FoF-scale density radius (length units); 0 = off
+    int slab_x0, slab_nx;        // sink slabs: x cell indices [x0, x0 + nx) periodic; nx = cpd: all
     int64_t ncell, ncol;
     NfParams prm;
     // options

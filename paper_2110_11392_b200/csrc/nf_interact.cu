@@ -61,10 +61,18 @@ __device__ __forceinline__ float mufu_rsq(float x) {
 // ------------------------------------------------------------------------------ A4: scheduler
 // Sink work items: every z-column (cx,cy) is cut into blocks of consecutive PADDED grid-order
 // slots, balanced within the column ("sink particles are arranged into blocks").
-__global__ void __launch_bounds__(256) k_col_blocks(int ncol, int cpd, const uint32_t *__restrict__ poff, uint32_t *__restrict__ col_nblk) {
+// sink slabs: only columns whose x cell index lies in the periodic range [x0, x0 + nx) hold sinks
+// (slab decomposition); the other columns are sources only (ghost slabs).
+__device__ __forceinline__ bool nf_sink_slab(int cx, int cpd, int x0, int nx) {
+    int d = cx - x0;
+    if (d < 0) d += cpd;
+    return d < nx;
+}
+__global__ void __launch_bounds__(256) k_col_blocks(int ncol, int cpd, int x0, int nx, const uint32_t *__restrict__ poff, uint32_t *__restrict__ col_nblk) {
     int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= ncol) return;
     uint32_t n = poff[(col + 1) * cpd] - poff[col * cpd];
+    if (!nf_sink_slab(col / cpd, cpd, x0, nx)) n = 0;
     col_nblk[col] = (n + NF_BS - 1) / NF_BS;
 }
 
@@ -172,7 +180,7 @@ nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st) {
         k_choose_rc<<<1, 32, 0, st>>>(sum2, (double)N, plummer ? ep : ctx->prm.eps_cells, plummer ? ep * ep : 0.0, ctx->opt_rc,
                                       (float *)(ctx->d_ctrl + 96)); ctx->launches++;
     }
-    k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk); ctx->launches++;
+    k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->slab_x0, ctx->slab_nx, ctx->d_poff, ctx->d_col_nblk); ctx->launches++;
     nf_status rc = nf_scan_u32(ctx, ctx->d_col_nblk, (uint32_t)ncol, ctx->d_col_base, st);
     if (rc != NF_OK) return rc;
     k_fill_blocks<<<(ncol + 127) / 128, 128, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk, ctx->d_col_base, ctx->d_blk, ctx->R); ctx->launches++;
@@ -789,14 +797,15 @@ nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st) {
     return NF_OK;
 }
 
-// pairs = sum_c n_c * sum_{c' in N(c)} n_c'   (the caller subtracts N)
-__global__ void __launch_bounds__(256) k_paircount(int cpd, int R, const uint32_t *__restrict__ offsets, unsigned long long *__restrict__ out) {
+// out[0] = sum over sink cells c of n_c * sum_{c' in N(c)} n_c', out[1] = number of sinks (the caller subtracts it)
+__global__ void __launch_bounds__(256) k_paircount(int cpd, int R, int x0, int nx, const uint32_t *__restrict__ offsets, unsigned long long *__restrict__ out) {
     const int ncell = cpd * cpd * cpd;
     int c = blockIdx.x * blockDim.x + threadIdx.x;
-    unsigned long long v = 0;
+    unsigned long long v = 0, ns = 0;
     if (c < ncell) {
         const unsigned long long nc = offsets[c + 1] - offsets[c];
-        if (nc) {
+        if (nc && nf_sink_slab(c / (cpd * cpd), cpd, x0, nx)) {
+            ns = nc;
             const int ck = c % cpd, cj = (c / cpd) % cpd, ci = c / (cpd * cpd);
             unsigned long long s = 0;
             for (int a = -R; a <= R; ++a) {
@@ -814,14 +823,14 @@ __global__ void __launch_bounds__(256) k_paircount(int cpd, int R, const uint32_
         }
     }
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-    if ((threadIdx.x & 31) == 0 && v) atomicAdd(out, v);
+    for (int d = 16; d > 0; d >>= 1) { v += __shfl_xor_sync(0xffffffffu, v, d); ns += __shfl_xor_sync(0xffffffffu, ns, d); }
+    if ((threadIdx.x & 31) == 0 && ns) { atomicAdd(out, v); atomicAdd(out + 1, ns); }
 }
 
 nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st) {
-    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_pairs, 0, sizeof(unsigned long long), st));
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_pairs, 0, 2 * sizeof(unsigned long long), st));
     const int ncell = (int)ctx->ncell;
-    k_paircount<<<(ncell + 255) / 256, 256, 0, st>>>(ctx->cpd, ctx->R, ctx->d_offsets, ctx->d_pairs); ctx->launches++;
+    k_paircount<<<(ncell + 255) / 256, 256, 0, st>>>(ctx->cpd, ctx->R, ctx->slab_x0, ctx->slab_nx, ctx->d_offsets, ctx->d_pairs); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }

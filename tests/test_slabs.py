@@ -1,0 +1,195 @@
+"""x-slab decomposition (paper_2110_11392_b200/slabs.py): host logic on CPU, the halo exchange
+over gloo with world_size 2, and (GPU) a decomposition emulated rank by rank on one device
+against the single-call result and the oracle."""
+import json
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2110_11392_b200 import slabs
+from paper_2110_11392_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+# ----------------------------------------------------------------------------- host logic (CPU)
+def test_slab_and_cell_index_match_the_oracle_binning(oracle_mod):
+    rng = np.random.default_rng(0)
+    pos = rng.random((5000, 3)).astype(np.float32)
+    pos[:5, 0] = [0.0, np.nextafter(np.float32(1.0), np.float32(0.0)), 1.0 / 7, 2.0 / 7, 0.999999]
+    cell, _ = oracle_mod.bin_particles(pos, 7)
+    t = torch.from_numpy(pos)
+    assert np.array_equal(slabs.cell_index(t, 7).numpy(), cell)
+    assert np.array_equal(slabs.slab_index(t, 7).numpy(), cell // 49)
+
+
+def test_pairs_per_slab_is_the_pair_count_identity(oracle_mod):
+    cfg = W.scaled(W.CONFIGS[3], 9)
+    pos = W.make_positions(cfg)
+    cell, _ = oracle_mod.bin_particles(pos, cfg.cpd)
+    offsets, _ = oracle_mod.cell_lists(cell, cfg.cpd)
+    counts = torch.from_numpy(np.diff(offsets))
+    per = slabs.pairs_per_slab(counts, cfg.cpd, cfg.R)
+    assert int(per.sum()) - cfg.N == oracle_mod.pair_count(offsets, cfg.cpd, cfg.R)
+    # brute force for one slab
+    n = np.diff(offsets).reshape(cfg.cpd, cfg.cpd, cfg.cpd)
+    x, tot = 4, 0
+    for j in range(cfg.cpd):
+        for k in range(cfg.cpd):
+            for a in range(-cfg.R, cfg.R + 1):
+                for b in range(-cfg.R, cfg.R + 1):
+                    for c in range(-cfg.R, cfg.R + 1):
+                        tot += n[x, j, k] * n[(x + a) % cfg.cpd, (j + b) % cfg.cpd, (k + c) % cfg.cpd]
+    assert int(per[x]) == tot
+
+
+@pytest.mark.parametrize("world", [1, 2, 3, 4, 8])
+def test_balance_slabs_covers_and_balances(world):
+    rng = np.random.default_rng(world)
+    work = torch.from_numpy(rng.integers(1, 1000, size=35))
+    b = slabs.balance_slabs(work, world)
+    assert len(b) == world and b[0][0] == 0 and sum(nx for _, nx in b) == 35 and all(nx >= 1 for _, nx in b)
+    for (x0, nx), (x1, _) in zip(b, b[1:]):
+        assert x0 + nx == x1
+    share = [int(work[x0:x0 + nx].sum()) for x0, nx in b]
+    assert max(share) <= int(work.sum()) / world + int(work.max())          # within one slab of the ideal
+    # degenerate: all the work in one slab still leaves every rank a slab
+    w2 = torch.zeros(9, dtype=torch.int64)
+    w2[3] = 100
+    b2 = slabs.balance_slabs(w2, min(world, 9))
+    assert all(nx >= 1 for _, nx in b2) and sum(nx for _, nx in b2) == 9
+    with pytest.raises(ValueError):
+        slabs.balance_slabs(torch.ones(3), 4)
+
+
+@pytest.mark.parametrize("cpd,R,world", [(35, 2, 2), (35, 2, 8), (9, 2, 3), (7, 3, 2), (5, 2, 2), (6, 2, 6)])
+def test_halo_and_send_plans_are_consistent(cpd, R, world):
+    work = torch.ones(cpd)
+    b = slabs.balance_slabs(work, world)
+    own = slabs.owner_of_slab(b, cpd)
+    for r in range(world):
+        need = slabs.halo_slabs(b, cpd, R, r)
+        x0, nx = b[r]
+        mine = {(x0 + i) % cpd for i in range(nx)}
+        expect = {(x + d) % cpd for x in mine for d in range(-R, R + 1)} - mine
+        assert set(need) == expect and len(need) == len(set(need))
+        # what the others send to r is exactly what r needs
+        got = []
+        for q in range(world):
+            got += slabs.send_plan(b, cpd, R, q).get(r, [])
+        assert sorted(got) == sorted(need)
+        assert all(own[x] != r for x in need)
+
+
+def test_local_with_ghosts_selects_own_and_halo():
+    cfg = W.scaled(W.CONFIGS[2], 9)
+    pos = torch.from_numpy(W.make_positions(cfg))
+    b = slabs.balance_slabs(torch.ones(9), 3)
+    xs = slabs.slab_index(pos, 9)
+    tot = 0
+    for r in range(3):
+        own, ghost = slabs.local_with_ghosts(pos, b, 9, 2, r)
+        x0, nx = b[r]
+        assert bool((torch.remainder(slabs.slab_index(own, 9) - x0, 9) < nx).all())
+        need = set(slabs.halo_slabs(b, 9, 2, r))
+        assert set(slabs.slab_index(ghost, 9).tolist()) <= need
+        assert ghost.shape[0] == int(sum((xs == x).sum() for x in need))
+        tot += own.shape[0]
+    assert tot == cfg.N
+
+
+_WORKER = r'''
+import os, sys, json
+sys.path.insert(0, os.environ["NF_ROOT"])
+import numpy as np, torch
+import torch.distributed as dist
+from paper_2110_11392_b200 import slabs, workloads as W
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+cfg = W.scaled(W.CONFIGS[3], 9)
+pos = torch.from_numpy(W.make_positions(cfg))            # every rank generates the same seeded set
+counts = torch.bincount(slabs.cell_index(pos, cfg.cpd), minlength=cfg.cpd ** 3)
+bounds = slabs.balance_slabs(slabs.pairs_per_slab(counts, cfg.cpd, cfg.R), world)
+own, ghost_expect = slabs.local_with_ghosts(pos, bounds, cfg.cpd, cfg.R, rank)
+ghost = slabs.halo_exchange(own, slabs.slab_index(own, cfg.cpd), bounds, cfg.cpd, cfg.R)
+key = lambda t: np.sort(np.ascontiguousarray(t.numpy()).view([("x", "f4"), ("y", "f4"), ("z", "f4")]).ravel(), order=["x", "y", "z"])
+ok = ghost.shape == ghost_expect.shape and np.array_equal(key(ghost), key(ghost_expect))
+res = torch.tensor([int(ok), own.shape[0], ghost.shape[0]])
+out = [torch.zeros_like(res) for _ in range(world)]
+dist.all_gather(out, res)
+if rank == 0:
+    print(json.dumps({"ok": [int(o[0]) for o in out], "own": [int(o[1]) for o in out], "ghost": [int(o[2]) for o in out],
+                      "N": cfg.N, "bounds": bounds}))
+dist.destroy_process_group()
+'''
+
+
+def test_halo_exchange_two_gloo_ranks(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER)
+    env = dict(os.environ, NF_ROOT=ROOT)
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29741", str(script)],
+                         capture_output=True, text=True, env=env, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    r = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert r["ok"] == [1, 1] and sum(r["own"]) == r["N"] and all(g > 0 for g in r["ghost"])
+    assert sum(nx for _, nx in r["bounds"]) == 9
+
+
+# ----------------------------------------------------------------------------- GPU: emulated decomposition
+@pytest.mark.gpu
+@pytest.mark.parametrize("label,cfg,world", [("cfg2@13 x3", W.scaled(W.CONFIGS[2], 13), 3),
+                                             ("cfg3@10 x4", W.scaled(W.CONFIGS[3], 10), 4),
+                                             ("cfg5@9 R3 x2", W.scaled(W.CONFIGS[5], 9), 2),
+                                             ("cfg2@5 (=2R+1) x2", W.scaled(W.CONFIGS[2], 5), 2)])
+def test_emulated_slab_decomposition_matches_single_call_and_oracle(oracle_mod, label, cfg, world):
+    """Ranks run one after the other on one GPU (no kernel waits on another: see the profiling
+    guide): each takes its own slabs + ghosts, calls nf_accel with nf_set_sink_slabs, and the
+    union must equal the undecomposed result within the parity bar; pair counts add up exactly."""
+    from paper_2110_11392_b200.binding import NearField
+    assert torch.cuda.is_available()
+    pos_np = W.make_positions(cfg)
+    pos = torch.from_numpy(pos_np).cuda()
+    ref, ref_pairs = oracle_mod.accel(pos_np, cfg.cpd, cfg.R, cfg.eps_p)
+    counts = torch.bincount(slabs.cell_index(pos, cfg.cpd), minlength=cfg.cpd ** 3)
+    bounds = slabs.balance_slabs(slabs.pairs_per_slab(counts, cfg.cpd, cfg.R), world)
+    xs = slabs.slab_index(pos, cfg.cpd)
+    got = torch.full_like(pos, float("nan"))
+    pairs = 0
+    for r in range(world):
+        own, ghost = slabs.local_with_ghosts(pos, bounds, cfg.cpd, cfg.R, r)
+        x0, nx = bounds[r]
+        idx = torch.nonzero(torch.remainder(xs - x0, cfg.cpd) < nx).ravel()
+        allp = torch.cat([own, ghost]).contiguous()
+        with NearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+            nf.set_gm(1.0 / cfg.N)                       # the global G*m, not 1/(own + ghost)
+            nf.set_sink_slabs(x0, nx)
+            acc = torch.full_like(allp, float("nan"))
+            nf.accel(allp, acc)
+            nf.sync()
+            pairs += nf.interaction_count()
+            assert bool(torch.isnan(acc[own.shape[0]:]).all())       # ghost rows are left untouched
+            got[idx] = acc[: own.shape[0]]
+    assert pairs == ref_pairs
+    g = got.cpu().numpy().astype(np.float64)
+    d = np.linalg.norm(g - ref, axis=1)
+    a = np.linalg.norm(ref, axis=1)
+    rms = np.sqrt((a ** 2).mean())
+    assert np.isfinite(g).all()
+    assert d.max() <= 1e-5 * rms, f"{label}: {d.max() / rms:.3e}"
+    assert np.median(d[a > 0] / a[a > 0]) <= 2e-6
+
+
+@pytest.mark.gpu
+def test_sink_slab_setter_rejects_bad_ranges():
+    from paper_2110_11392_b200.binding import NearField, NearFieldError
+    with NearField(7, 2, 1e-3, 1.0) as nf:
+        for x0, nx in ((-1, 3), (7, 1), (0, 0), (0, 8)):
+            with pytest.raises(NearFieldError):
+                nf.set_sink_slabs(x0, nx)
+        nf.set_sink_slabs(6, 7)
