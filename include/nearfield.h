@@ -129,6 +129,17 @@ nf_status nf_set_sink_slabs(nf_ctx *ctx, int x0, int nx);
 nf_status nf_accel4(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc4, void *cuda_stream);
 
 /*
+ * nf_accel_f64 -- the paper's "Double precision: yes" build (Fig. 19) as a second
+ * entry point, for validating the float32 kernel on the GPU: the same
+ * binning, then a plain direct sum in double precision (offsets recomputed in double from the
+ * float32 positions, piecewise law with a branch, no packed arithmetic, no close-pair path).
+ *   d_acc [out] device, N*3 DOUBLES, input order.  Honours nf_set_gm, nf_set_softening and
+ *   nf_set_sink_slabs.  Some 30 times slower than nf_accel; not part of the timed path.
+ * Errors as nf_accel.
+ */
+nf_status nf_accel_f64(nf_ctx *ctx, const float *d_pos, int64_t N, double *d_acc, void *cuda_stream);
+
+/*
  * nf_accel_host -- the same through HOST buffers: copies h_pos to the device, runs
  * nf_accel, copies the result back into h_acc and synchronises (this is the end-to-end
  * call bench.py times; pinned host memory makes the copies asynchronous DMA).

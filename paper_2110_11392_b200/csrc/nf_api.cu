@@ -207,6 +207,24 @@ extern "C" nf_status nf_accel4(nf_ctx *c, const float *d_pos, int64_t N, float *
     return accel_any(c, d_pos, N, d_acc4, 4, cuda_stream);
 }
 
+extern "C" nf_status nf_accel_f64(nf_ctx *c, const float *d_pos, int64_t N, double *d_acc, void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N < 0 || (N > 0 && (!d_pos || !d_acc)) || (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_accel_f64: bad argument (N=%lld)", (long long)N);
+        return NF_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (N == 0) return NF_OK;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    nf_status rc = ensure_scratch(c, N);
+    if (rc != NF_OK) return rc;
+    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    rc = nf_run_binner(c, d_pos, N, st);
+    if (rc != NF_OK) return rc;
+    return nf_run_f64(c, d_pos, N, d_acc, st);
+}
+
 extern "C" nf_status nf_sync(nf_ctx *c) {
     if (!c) return NF_EINVAL;
     if (!c->have_last) return NF_OK;

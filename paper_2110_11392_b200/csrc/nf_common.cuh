@@ -84,7 +84,7 @@ struct nf_ctx {
     uint32_t *d_col_nblk, *d_col_base, *d_scan32_blk, *d_blk_order;
     NfBlockDesc *d_blk;
     uint32_t *d_ctrl;            // [0] work counter  [1] number of blocks  [2] bad-position flag  [3] npad
-                                 // [16..79] cost histogram  [96..98] float rc^2, rc, rc^-3  [100..101] u64 sum n_c^2
+                                 // [16..79] cost histogram  [96..98] float rc^2, rc, rc^-3  [100..101] u64 sum n_c^2  [104] work counter of nf_accel_f64
     unsigned long long *d_pairs;
     int32_t *d_nbr;              // debug neighbour list
     // host staging for nf_accel_host
@@ -115,6 +115,7 @@ nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st);
 nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st);
 nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st);
+nf_status nf_run_f64(nf_ctx *ctx, const float *d_pos, int64_t N, double *d_acc, cudaStream_t st);
 nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_interact_setup(nf_ctx *ctx);
 nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st);
