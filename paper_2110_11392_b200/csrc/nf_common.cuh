@@ -20,6 +20,10 @@
 #ifndef NF_NW
 #define NF_NW 4                   // consumer warps per CTA
 #endif
+#ifndef NF_PRODUCER_WARP
+#define NF_PRODUCER_WARP 1        // 1: a dedicated producer warp per CTA; 0: consumer warp 0 also fills the ring
+#endif
+#define NF_CTA_THREADS ((NF_NW + NF_PRODUCER_WARP) * 32)
 #ifndef NF_SINKS
 #define NF_SINKS 2                // sinks per consumer thread (adjacent slots 2t, 2t+1 of the warp's range when 2)
 #endif

@@ -39,6 +39,14 @@ __device__ __forceinline__ bool mbar_try(uint64_t *bar, uint32_t parity) {
         "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     return ok != 0u;
 }
+__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {     // non-blocking
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0u;
+}
 // SLEEP_NS > 0: back off between polls so that a waiting warp does not take issue slots from
 // the working warps of its SM sub-partition (the producer is always several stages ahead).
 template <int SLEEP_NS>
@@ -219,6 +227,12 @@ struct __align__(128) Stage {
     float zs[NF_TILE];
     uint32_t tab[NF_TABMAX + 1];
     StageHdr hdr;
+};
+
+struct ProdState {       // cursor of the stage producer (block, column, z-run, chunk), kept in shared memory
+    int mode;            // 0 next block, 1 next z-run, 2 next chunk of the run, 3 end of block, 4 finished
+    int flags, a, b, u, U1, Z1, ci, cj, ucur, run;
+    uint32_t col, s0, cnt, c0, ge;
 };
 
 struct InteractArgs {
@@ -434,7 +448,7 @@ __device__ __forceinline__ void fold(float &tot, float &comp, float v, int kahan
 // LAW: NF_SOFT_SPLINE (Eq. 3) or NF_SOFT_PLUMMER (Eq. 2).  DENS: also accumulate the FoF-scale density
 // estimate in the near cells and store it as the 4th output component.
 template <bool FLAG, int LAW, bool DENS>
-__global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(const InteractArgs A) {
+__global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const InteractArgs A) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Stage *stages = reinterpret_cast<Stage *>(smem_raw);
     __shared__ uint64_t full_bar[NF_NSTAGE], empty_bar[NF_NSTAGE];
@@ -458,6 +472,7 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
     int stage = 0;
     uint32_t phase = 0;
 
+#if NF_PRODUCER_WARP
     if (warp == NF_NW) {
         // =========================== producer warp ===========================================
         const uint32_t nblocks = A.ctrl[1];
@@ -537,6 +552,109 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
         emit(NF_F_EXIT, 0, 0, 0, 0, 0u, 0u, 0, 0u, 0u, 0u);
         return;
     }
+#else
+    // =========================== production by consumer warp 0 ================================
+    // No dedicated producer warp: its registers go to the consumers (4 CTAs x 4 warps x 128
+    // registers fill the register file).  Warp 0 refills freed ring slots at its stage
+    // boundaries; the (block, column, z-run, chunk) cursor lives in shared memory so that it costs
+    // no registers in the pair loop.  produce_one() emits exactly one stage.
+    __shared__ ProdState ps;
+    __shared__ uint32_t ptab[32];
+    if (threadIdx.x == 0) { ps.mode = 0; ps.flags = 0; }
+    __syncthreads();
+    int pstage = 0, ahead = 0;
+    uint32_t pphase = 0;
+    bool pdone = false;
+    auto produce_one = [&]() -> bool {
+        Stage &S = stages[pstage];
+        uint64_t *fb = &full_bar[pstage];
+        auto emit = [&](int flags, int a, int b, int zu0, int nc, uint32_t tabval, uint32_t g_lo, int g_cnt, uint32_t col, uint32_t s0, uint32_t cnt) {
+            S.tab[lane] = tabval;
+            if (lane == 0) {
+                StageHdr h;
+                h.flags = flags; h.a = a; h.b = b; h.zu0 = zu0; h.nc = nc; h.g_lo = g_lo; h.g_cnt = g_cnt;
+                h.col = col; h.s0 = s0; h.cnt = cnt; h.pad0 = 0; h.pad1 = 0;
+                S.hdr = h;
+            }
+            __syncwarp();
+            if (lane == 0) {
+                if (g_cnt > 0) {
+                    const uint32_t bytes = (uint32_t)g_cnt * 4u;
+                    mbar_arrive_expect_tx(fb, 3u * bytes);
+                    bulk_g2s(S.xs, A.sx + g_lo, bytes, fb);
+                    bulk_g2s(S.ys, A.sy + g_lo, bytes, fb);
+                    bulk_g2s(S.zs, A.sz + g_lo, bytes, fb);
+                } else {
+                    mbar_arrive(fb);
+                }
+            }
+        };
+        ProdState q = ps;
+        bool last = false;
+        for (;;) {
+            if (q.mode == 0) {                       // next sink block
+                uint32_t w = 0;
+                if (lane == 0) w = atomicAdd(&A.ctrl[0], 1u);
+                w = __shfl_sync(0xffffffffu, w, 0);
+                if (w >= A.ctrl[1]) { emit(NF_F_EXIT, 0, 0, 0, 0, 0u, 0u, 0, 0u, 0u, 0u); q.mode = 4; last = true; break; }
+                const NfBlockDesc d = A.blk[A.order[w]];
+                if (d.cnt == 0) continue;
+                q.col = d.col; q.s0 = d.s0; q.cnt = d.cnt;
+                q.ci = (int)(d.col / (uint32_t)cpd); q.cj = (int)(d.col % (uint32_t)cpd);
+                const int colbase = (int)d.col * cpd;
+                q.Z1 = (int)(A.skey[d.s0] & ~NF_PAD_FLAG) - colbase;
+                q.U1 = (int)(A.skey[d.s0 + d.cnt - 1] & ~NF_PAD_FLAG) - colbase + R;
+                q.a = -R; q.b = -R; q.u = q.Z1 - R; q.flags = NF_F_NEWBLOCK; q.mode = 1;
+            }
+            if (q.mode == 1) {                       // next non-empty z-run of column (a, b)
+                if (q.u > q.U1) {
+                    q.u = q.Z1 - R;
+                    if (++q.b > R) { q.b = -R; ++q.a; }
+                    if (q.a > R) { q.mode = 3; continue; }
+                }
+                int ia; const int sci = nf_wrap1(q.ci + q.a, cpd, ia);
+                int ib; const int scj = nf_wrap1(q.cj + q.b, cpd, ib);
+                const int cb = (sci * cpd + scj) * cpd;
+                const int wz = nf_mod(q.u, cpd);
+                int run = q.U1 - q.u + 1;
+                if (run > cpd - wz) run = cpd - wz;
+                if (run > NF_TABMAX) run = NF_TABMAX;
+                // table: padded offsets of cells wz .. wz+run (run+1 entries)
+                const uint32_t tv = A.poff[cb + wz + (lane <= run ? lane : run)];
+                const uint32_t g0 = __shfl_sync(0xffffffffu, tv, 0);
+                const uint32_t g1 = __shfl_sync(0xffffffffu, tv, run);
+                q.ucur = q.u; q.run = run;
+                q.u += run;
+                if (g1 <= g0) continue;
+                q.c0 = g0 & ~3u; q.ge = (g1 + 3u) & ~3u;
+                ptab[lane] = tv;
+                __syncwarp();
+                q.mode = 2;
+            }
+            if (q.mode == 2) {                       // next chunk of the run
+                const uint32_t c1 = (q.c0 + NF_TILE < q.ge) ? q.c0 + NF_TILE : q.ge;
+                // table entry = first slot of the cell relative to this stage, clamped to the stage
+                int tl = (int)(ptab[lane] - q.c0);
+                const int tc = (int)(c1 - q.c0);
+                tl = tl < 0 ? 0 : (tl > tc ? tc : tl);
+                emit(q.flags, q.a, q.b, q.ucur, q.run, (uint32_t)tl, q.c0, tc, q.col, q.s0, q.cnt);
+                q.flags = 0;
+                q.c0 += NF_TILE;
+                if (q.c0 >= q.ge) q.mode = 1;
+                break;
+            }
+            if (q.mode == 3) {                       // end of the block
+                emit(q.flags | NF_F_LAST, 0, 0, 0, 0, 0u, 0u, 0, q.col, q.s0, q.cnt);
+                q.mode = 0;
+                break;
+            }
+        }
+        if (lane == 0) ps = q;
+        __syncwarp();
+        return last;
+    };
+
+#endif
 
     // =============================== consumer warps ==========================================
     // Thread t of warp w holds the kS sinks at slots s0 + (32 w + t) kS + j of the block (adjacent
@@ -558,6 +676,19 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
     const int W = 2 * R + 1;
 
     for (;;) {
+#if !NF_PRODUCER_WARP
+        if (warp == 0 && !pdone) {
+            // refill every free slot; block only when there is nothing left to consume
+            while (ahead < NF_NSTAGE) {
+                if (ahead > 0) { if (!mbar_test(&empty_bar[pstage], pphase ^ 1u)) break; }
+                else mbar_wait<0>(&empty_bar[pstage], pphase ^ 1u);
+                pdone = produce_one();
+                if (++pstage == NF_NSTAGE) { pstage = 0; pphase ^= 1u; }
+                ++ahead;
+                if (pdone) break;
+            }
+        }
+#endif
         Stage &S = stages[stage];
         mbar_wait<NF_CONSUMER_SLEEP_NS>(&full_bar[stage], phase);
         const int flags = S.hdr.flags;
@@ -703,6 +834,9 @@ __global__ void __launch_bounds__((NF_NW + 1) * 32, NF_MIN_CTAS) k_interact(cons
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty_bar[stage]);
         if (++stage == NF_NSTAGE) { stage = 0; phase ^= 1u; }
+#if !NF_PRODUCER_WARP
+        --ahead;
+#endif
     }
 }
 
@@ -728,7 +862,7 @@ nf_status nf_interact_setup(nf_ctx *ctx) {
                 InteractKernel k = interact_kernel(law, dens, flag);
                 NF_CUDA_OK(ctx, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                 int n1 = 0;
-                NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n1, k, (NF_NW + 1) * 32, smem));
+                NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n1, k, NF_CTA_THREADS, smem));
                 if (n1 < nb) nb = n1;
             }
     if (nb < 1) { snprintf(ctx->err, sizeof(ctx->err), "interaction kernel does not fit on an SM"); return NF_ECUDA; }
@@ -761,7 +895,7 @@ nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_o
     A.near_cheb = nc;
     const int grid = ctx->sm_count * g_interact_blocks_per_sm;
     for (int flag = 1; flag >= 0; --flag) {     // the instantiation whose regime is not in force returns at once
-        interact_kernel(law, dens, flag)<<<grid, (NF_NW + 1) * 32, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
+        interact_kernel(law, dens, flag)<<<grid, NF_CTA_THREADS, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
     }
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
