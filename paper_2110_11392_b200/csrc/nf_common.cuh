@@ -21,7 +21,7 @@
 #define NF_NW 4                   // consumer warps per CTA
 #endif
 #ifndef NF_PRODUCER_WARP
-#define NF_PRODUCER_WARP 1        // 1: a dedicated producer warp per CTA; 0: consumer warp 0 also fills the ring
+#define NF_PRODUCER_WARP 0        // 1: a dedicated producer warp per CTA; 0: consumer warp 0 also fills the ring
 #endif
 #define NF_CTA_THREADS ((NF_NW + NF_PRODUCER_WARP) * 32)
 #ifndef NF_SINKS
@@ -36,7 +36,7 @@
 #endif
 #define NF_TABMAX 31              // source cells per segment table (32 entries = one per producer lane)
 #ifndef NF_NSTAGE
-#define NF_NSTAGE 7               // pipeline depth
+#define NF_NSTAGE 4               // pipeline depth
 #endif
 #ifndef NF_CELL_PAD
 #define NF_CELL_PAD 4             // every cell is padded to a multiple of this many slots (power of two, >= 2)
@@ -44,7 +44,7 @@
 #ifndef NF_UNROLL
 #endif
 #ifndef NF_MIN_CTAS
-#define NF_MIN_CTAS 3             // resident CTAs per SM the interaction kernel is compiled for
+#define NF_MIN_CTAS 4             // resident CTAs per SM the interaction kernel is compiled for
 #endif
 #ifndef NF_PRODUCER_SLEEP_NS
 #define NF_PRODUCER_SLEEP_NS 0    // back-off of the producer warp while its ring slot is still in use
