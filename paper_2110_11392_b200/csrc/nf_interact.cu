@@ -230,7 +230,7 @@ struct __align__(128) Stage {
 };
 
 struct ProdState {       // cursor of the stage producer (block, column, z-run, chunk), kept in shared memory
-    int mode;            // 0 next block, 1 next z-run, 2 next chunk of the run, 3 end of block, 4 finished
+    int mode;            // 0 next block, 1 next z-run, 5 z-run requested, 2 next chunk of the run, 3 end of block, 4 finished
     int flags, a, b, u, U1, Z1, ci, cj, ucur, run;
     uint32_t col, s0, cnt, c0, ge;
 };
@@ -565,6 +565,27 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
     int pstage = 0, ahead = 0;
     uint32_t pphase = 0;
     bool pdone = false;
+    uint32_t tvp = 0;        // table entry of the requested run (lane l: padded offset of its cell l), in flight between calls
+    // advance the cursor to the next z-run of the block's source columns and request its table
+    // (padded offsets of cells wz .. wz+run); mode 5 = requested, mode 3 = the block has no more runs
+    auto issue_run = [&](ProdState &q) {
+        if (q.u > q.U1) {
+            q.u = q.Z1 - R;
+            if (++q.b > R) { q.b = -R; ++q.a; }
+            if (q.a > R) { q.mode = 3; return; }
+        }
+        int ia; const int sci = nf_wrap1(q.ci + q.a, cpd, ia);
+        int ib; const int scj = nf_wrap1(q.cj + q.b, cpd, ib);
+        const int cb = (sci * cpd + scj) * cpd;
+        const int wz = nf_mod(q.u, cpd);
+        int run = q.U1 - q.u + 1;
+        if (run > cpd - wz) run = cpd - wz;
+        if (run > NF_TABMAX) run = NF_TABMAX;
+        tvp = A.poff[cb + wz + (lane <= run ? lane : run)];
+        q.ucur = q.u; q.run = run;
+        q.u += run;
+        q.mode = 5;
+    };
     auto produce_one = [&]() -> bool {
         Stage &S = stages[pstage];
         uint64_t *fb = &full_bar[pstage];
@@ -606,28 +627,13 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                 q.U1 = (int)(A.skey[d.s0 + d.cnt - 1] & ~NF_PAD_FLAG) - colbase + R;
                 q.a = -R; q.b = -R; q.u = q.Z1 - R; q.flags = NF_F_NEWBLOCK; q.mode = 1;
             }
-            if (q.mode == 1) {                       // next non-empty z-run of column (a, b)
-                if (q.u > q.U1) {
-                    q.u = q.Z1 - R;
-                    if (++q.b > R) { q.b = -R; ++q.a; }
-                    if (q.a > R) { q.mode = 3; continue; }
-                }
-                int ia; const int sci = nf_wrap1(q.ci + q.a, cpd, ia);
-                int ib; const int scj = nf_wrap1(q.cj + q.b, cpd, ib);
-                const int cb = (sci * cpd + scj) * cpd;
-                const int wz = nf_mod(q.u, cpd);
-                int run = q.U1 - q.u + 1;
-                if (run > cpd - wz) run = cpd - wz;
-                if (run > NF_TABMAX) run = NF_TABMAX;
-                // table: padded offsets of cells wz .. wz+run (run+1 entries)
-                const uint32_t tv = A.poff[cb + wz + (lane <= run ? lane : run)];
-                const uint32_t g0 = __shfl_sync(0xffffffffu, tv, 0);
-                const uint32_t g1 = __shfl_sync(0xffffffffu, tv, run);
-                q.ucur = q.u; q.run = run;
-                q.u += run;
-                if (g1 <= g0) continue;
+            if (q.mode == 1) issue_run(q);           // (only right after a block start or an empty run: not prefetched)
+            if (q.mode == 5) {                       // the run's table has been requested: is the run non-empty?
+                const uint32_t g0 = __shfl_sync(0xffffffffu, tvp, 0);
+                const uint32_t g1 = __shfl_sync(0xffffffffu, tvp, q.run);
+                if (g1 <= g0) { q.mode = 1; continue; }
                 q.c0 = g0 & ~3u; q.ge = (g1 + 3u) & ~3u;
-                ptab[lane] = tv;
+                ptab[lane] = tvp;
                 __syncwarp();
                 q.mode = 2;
             }
@@ -640,7 +646,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                 emit(q.flags, q.a, q.b, q.ucur, q.run, (uint32_t)tl, q.c0, tc, q.col, q.s0, q.cnt);
                 q.flags = 0;
                 q.c0 += NF_TILE;
-                if (q.c0 >= q.ge) q.mode = 1;
+                if (q.c0 >= q.ge) { q.mode = 1; issue_run(q); }     // request the next run's table now, use it at the next call
                 break;
             }
             if (q.mode == 3) {                       // end of the block
