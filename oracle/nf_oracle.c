@@ -347,3 +347,45 @@ int64_t nfo_accel_variant(const float *pos, int64_t N, int cpd, int R, double ep
     free(so); free(cell); free(off); free(offsets); free(order);
     return pairs;
 }
+
+/*
+ * Cell multipoles, Eq. 4 (sec. 3.3.2), in the complete basis of
+ * cml = (p+3)(p+2)(p+1)/6 values per cell:
+ *     M_{i,j,k}^{a,b,c} = sum_q x_q^a y_q^b z_q^c,   0 <= a <= p, 0 <= b <= p-a, 0 <= c <= p-a-b,
+ * (x_q, y_q, z_q) = displacement of particle q "from the origin of cell (i,j,k)" = its offset from
+ * the cell centre (nfo_bin, reading S5), in length units.  The loop nest is the paper's pseudo-code
+ * (garbled in the extraction; restored from Eq. 4): for each particle, mx runs over
+ * x^a, mxy over x^a y^b, mxyz over x^a y^b z^c by repeated multiplication, and M[a,b,c] += mxyz with
+ * (a,b,c) in that nesting order, which is also the order of the output index.
+ * M: ncell * cml doubles, cell-major (key = (cx*CPD+cy)*CPD+cz).  Particles of a cell are added in
+ * ascending input order.  Returns cml, or -1.
+ */
+int nfo_multipoles(const float *pos, int64_t N, int cpd, double box, int order, double *M) {
+    if (N < 0 || cpd < 1 || !(box > 0) || order < 0 || order > 16) return -1;
+    const int cml = (order + 3) * (order + 2) * (order + 1) / 6;
+    const int64_t ncell = (int64_t)cpd * cpd * cpd;
+    int32_t *cell = (int32_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int32_t));
+    double *off = (double *)malloc((size_t)(N > 0 ? N : 1) * 3 * sizeof(double));
+    if (!cell || !off || nfo_bin(pos, N, cpd, box, cell, off) != 0) { free(cell); free(off); return -1; }
+    memset(M, 0, (size_t)ncell * cml * sizeof(double));
+    for (int64_t q = 0; q < N; ++q) {
+        double *Mc = M + (size_t)cell[q] * cml;
+        const double X = off[3 * q], Y = off[3 * q + 1], Z = off[3 * q + 2];
+        int idx = 0;
+        double mx = 1.0;
+        for (int a = 0; a <= order; ++a) {
+            double mxy = mx;
+            for (int b = 0; b <= order - a; ++b) {
+                double mxyz = mxy;
+                for (int c = 0; c <= order - a - b; ++c) {
+                    Mc[idx++] += mxyz;
+                    mxyz *= Z;
+                }
+                mxy *= Y;
+            }
+            mx *= X;
+        }
+    }
+    free(cell); free(off);
+    return cml;
+}

@@ -70,6 +70,8 @@ def _load():
         L.nfo_pair_count.argtypes = [vp, i32, i32]
         L.nfo_accel.restype = i64
         L.nfo_accel.argtypes = [vp, i64, i32, i32, dbl, dbl, dbl, vp, i64, vp, i32]
+        L.nfo_multipoles.restype = i32
+        L.nfo_multipoles.argtypes = [vp, i64, i32, dbl, i32, vp]
         L.nfo_accel_variant.restype = i64
         L.nfo_accel_variant.argtypes = [vp, i64, i32, i32, dbl, dbl, dbl, i32, dbl, vp, i64, vp, vp, i32]
         _lib = L
@@ -179,3 +181,20 @@ def accel_variant(pos, cpd: int, R: int, eps_p: float, box: float = 1.0, gm: flo
     if pairs < 0:
         raise ValueError("nfo_accel_variant: bad arguments or non-finite position")
     return acc, dens, int(pairs)
+
+
+def multipoles(pos, cpd: int, order: int = 8, box: float = 1.0) -> np.ndarray:
+    """Cell multipoles of Eq. 4 in the complete basis -> float64 [cpd^3, cml],
+    cml = (p+3)(p+2)(p+1)/6, index order = the (a, b, c) nesting of the paper's pseudo-code."""
+    p = _f32pos(pos)
+    cml = (order + 3) * (order + 2) * (order + 1) // 6
+    M = np.zeros((cpd ** 3, cml), dtype=np.float64)
+    rc = _load().nfo_multipoles(p.ctypes.data, p.shape[0], cpd, float(box), int(order), M.ctypes.data)
+    if rc != cml:
+        raise ValueError("nfo_multipoles: bad arguments or non-finite position")
+    return M
+
+
+def multipole_index(order: int):
+    """the (a, b, c) triple of every column of ``multipoles`` (the pseudo-code's nesting order)"""
+    return [(a, b, c) for a in range(order + 1) for b in range(order - a + 1) for c in range(order - a - b + 1)]
