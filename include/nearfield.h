@@ -49,6 +49,7 @@ typedef enum {
 } nf_status;
 
 #define NF_MAX_R 4          /* compiled maximum near-field radius */
+#define NF_MAX_MULTIPOLE_ORDER 16   /* compiled maximum order p of nf_multipoles */
 #define NF_SOFT_SPLINE 0    /* Eq. 3, the paper's "single_spline" (Fig. 19) */
 #define NF_SOFT_PLUMMER 1   /* Eq. 2 */
 #define NF_N_STAGES 8       /* entries of nf_stage_ms */
@@ -138,6 +139,21 @@ nf_status nf_accel4(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc4, v
  * Errors as nf_accel.
  */
 nf_status nf_accel_f64(nf_ctx *ctx, const float *d_pos, int64_t N, double *d_acc, void *cuda_stream);
+
+/*
+ * nf_multipoles -- the cell multipoles of Eq. 4 (sec. 3.3.2), the particle-facing
+ * step of the far field that follows NearForce in the paper's pipeline, in the complete basis:
+ *     M_cell^{a,b,c} = sum over the particles q of the cell of x_q^a y_q^b z_q^c,
+ *     0 <= a <= order, 0 <= b <= order - a, 0 <= c <= order - a - b,
+ * (x_q, y_q, z_q) = offset of q from its cell centre in length units, in double precision.
+ *   d_M [out] device, cpd^3 * cml DOUBLES, cell-major (key = (cx*cpd+cy)*cpd+cz), cml =
+ *       (order+3)(order+2)(order+1)/6, element order = the nesting a (outer), b, c (inner) of the
+ *       paper's pseudo-code.  Empty cells get zeros.  order = 8 is the paper's choice.
+ * Runs the binning (A1-A3) of d_pos and one kernel; N == 0 zero-fills.  The conversion to the
+ * reduced basis, the FFTs and the convolution are not part of this library.
+ * NF_EINVAL: ctx/d_M NULL, d_pos NULL with N > 0, N < 0, order outside [0, NF_MAX_MULTIPOLE_ORDER].
+ */
+nf_status nf_multipoles(nf_ctx *ctx, const float *d_pos, int64_t N, int order, double *d_M, void *cuda_stream);
 
 /*
  * nf_accel_host -- the same through HOST buffers: copies h_pos to the device, runs

@@ -22,7 +22,7 @@ STAGE_NAMES = ["A1_key_hist", "A2_scan", "A3_scatter_rank_gather", "A4_scheduler
 SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", "nf_sync",
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
            "nf_interaction_count", "nf_probe_pipes", "nf_debug_read", "nf_launch_count", "nf_close_radius",
-           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64"]
+           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles"]
 
 
 class NearFieldError(RuntimeError):
@@ -55,6 +55,8 @@ def load_library() -> ctypes.CDLL:
     L.nf_accel4.argtypes = [vp, vp, i64, vp, vp]
     L.nf_set_softening.restype = i32
     L.nf_set_softening.argtypes = [vp, i32]
+    L.nf_multipoles.restype = i32
+    L.nf_multipoles.argtypes = [vp, vp, i64, i32, vp, vp]
     L.nf_accel_f64.restype = i32
     L.nf_accel_f64.argtypes = [vp, vp, i64, vp, vp]
     L.nf_set_sink_slabs.restype = i32
@@ -198,6 +200,20 @@ class NearField:
         self._check(_L.nf_accel_f64(self._h, pos.data_ptr() if N else None, N, acc.data_ptr() if N else None,
                                     ctypes.c_void_p(st.cuda_stream)))
         return acc
+
+    def multipoles(self, pos, order: int = 8, stream=None):
+        """nf_multipoles: Eq. 4 in the complete basis -> float64 [cpd^3, (p+3)(p+2)(p+1)/6] on the device."""
+        import torch
+        if not (pos.is_cuda and pos.dtype == torch.float32 and pos.is_contiguous() and pos.dim() == 2 and pos.shape[1] == 3):
+            raise ValueError("pos must be a contiguous CUDA float32 tensor of shape [N,3]")
+        N = pos.shape[0]
+        cml = (order + 3) * (order + 2) * (order + 1) // 6
+        M = torch.empty((self.cpd ** 3, max(cml, 1)), dtype=torch.float64, device=pos.device)
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        self._N = N
+        self._check(_L.nf_multipoles(self._h, pos.data_ptr() if N else None, N, int(order), M.data_ptr(),
+                                     ctypes.c_void_p(st.cuda_stream)))
+        return M
 
     def accel_ptr(self, d_pos: int, N: int, d_acc: int, cuda_stream: int = 0):
         """raw-pointer form of nf_accel (used by tests of the error paths)."""

@@ -225,6 +225,29 @@ extern "C" nf_status nf_accel_f64(nf_ctx *c, const float *d_pos, int64_t N, doub
     return nf_run_f64(c, d_pos, N, d_acc, st);
 }
 
+extern "C" nf_status nf_multipoles(nf_ctx *c, const float *d_pos, int64_t N, int order, double *d_M, void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N < 0 || !d_M || (N > 0 && !d_pos) || order < 0 || order > NF_MAX_MULTIPOLE_ORDER ||
+        (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_multipoles: bad argument (N=%lld order=%d)", (long long)N, order);
+        return NF_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    if (N == 0) {
+        const size_t cml = (size_t)(order + 3) * (order + 2) * (order + 1) / 6;
+        NF_CUDA_OK(c, cudaMemsetAsync(d_M, 0, (size_t)c->ncell * cml * sizeof(double), st));
+        return NF_OK;
+    }
+    nf_status rc = ensure_scratch(c, N);
+    if (rc != NF_OK) return rc;
+    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    rc = nf_run_binner(c, d_pos, N, st);
+    if (rc != NF_OK) return rc;
+    return nf_run_multipoles(c, d_pos, order, d_M, st);
+}
+
 extern "C" nf_status nf_sync(nf_ctx *c) {
     if (!c) return NF_EINVAL;
     if (!c->have_last) return NF_OK;
