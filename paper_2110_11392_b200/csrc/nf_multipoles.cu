@@ -8,15 +8,18 @@
 // values per cell, index order = the (a, b, c) nesting of the paper's pseudo-code.
 //
 // Mapping (the paper's AVX-512 metacode interleaves particles across vector lanes; here the
-// BASIS is spread across threads and the particles of the cell stream past it): one CTA of 64
-// threads per cell (160 for orders above 9); thread t owns one (a, b) pair (45 pairs at p = 8) and keeps its p-a-b+1
-// accumulators in registers; the particles of the cell are staged 32 at a time in shared memory
-// as (x, y, z) in double (offsets recomputed from the caller's float32 positions through the
-// grid-order permutation of A1-A3); per particle the thread forms x^a y^b z^c by the same
-// repeated multiplications as the pseudo-code and adds in ascending grid order, with explicit
-// __dmul_rn / __dadd_rn (no FMA contraction), so every element is the pseudo-code's value bit
-// for bit.  Bound: FP64 pipe (about 2 cml = 330 flop per 12-byte particle, against 3.2 GB of
-// output at config 4).
+// BASIS is spread across threads and the particles of the cell stream past it): one CTA per
+// cell, 64 threads up to order 9 (160 above); thread t owns one (a, b) pair -- pairs sorted by
+// descending element count p-a-b+1, so that the first warp holds the long ones and the second
+// warp's loop is short (p = 8: 45 pairs, warp bounds 9 and 2) -- and keeps its accumulators in
+// registers.  The particles of the cell are staged 32 at a time in shared memory as power
+// tables x^0..p, y^0..p, z^0..p in double (offsets recomputed from the caller's float32
+// positions through the grid-order permutation of A1-A3, powers by repeated multiplication as
+// in the pseudo-code); per particle a thread reads x^a and y^b (conflict-free multicast), forms
+// m = x^a y^b and does M[a,b,c] += m z^c as one FMA per element with z^c broadcast from shared
+// memory -- the FMA form the paper itself proposes ("M[a,b,c] += mxy*Zc[c]").
+// Particles are added in ascending grid order.  Bound: FP64 pipe (cml FMAs + (p+1)(p+2)/2
+// multiplies + 3p table multiplies per 12-byte particle, against 3.2 GB of output at config 4).
 #include "nf_common.cuh"
 
 #define NFM_TILE 32
@@ -32,58 +35,70 @@ struct MultipoleArgs {
     int ncell, order, cml;
 };
 
+// PMAX = compile-time bound of the order (8: the paper's choice; NFM_MAX_ORDER: any order)
+template <int PMAX>
 __global__ void __launch_bounds__(160) k_multipoles(const MultipoleArgs A) {
-    __shared__ double sx[NFM_TILE], sy[NFM_TILE], sz[NFM_TILE];
+    __shared__ double xp[NFM_TILE][PMAX + 1], yp[NFM_TILE][PMAX + 1], zp[NFM_TILE][PMAX + 1];
     const int p = A.order;
-    // thread t -> (a, b) in the nesting order of the basis, and the index of its first element
+    // thread t -> the t-th (a, b) pair in order of descending element count nc = p - a - b + 1
+    // (ties in basis order), and the index of the pair's first element in the basis order
     int a = 0, b = 0, base = 0, nc = 0;
     {
-        int t = (int)threadIdx.x, idx = 0;
-        bool found = false;
-        for (int aa = 0; aa <= p && !found; ++aa)
-            for (int bb = 0; bb <= p - aa; ++bb) {
-                if (t == 0) { a = aa; b = bb; base = idx; nc = p - aa - bb + 1; found = true; break; }
-                --t;
-                idx += p - aa - bb + 1;
-            }
-        if (!found) nc = 0;          // spare thread: only helps with the loads
+        int t = (int)threadIdx.x;
+        for (int want = p + 1; want >= 1 && nc == 0; --want) {       // pairs with a + b = p + 1 - want
+            int idx = 0;
+            for (int aa = 0; aa <= p && nc == 0; ++aa)
+                for (int bb = 0; bb <= p - aa; ++bb) {
+                    const int n = p - aa - bb + 1;
+                    if (n == want) {
+                        if (t == 0) { a = aa; b = bb; base = idx; nc = n; break; }
+                        --t;
+                    }
+                    idx += n;
+                }
+        }
     }
+    // longest element count in this warp (warp-uniform loop bound)
+    int ncw = nc;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) ncw = max(ncw, __shfl_xor_sync(0xffffffffu, ncw, d));
     for (int cell = blockIdx.x; cell < A.ncell; cell += gridDim.x) {
         const uint32_t p0 = A.offsets[cell], p1 = A.offsets[cell + 1];
-        double acc[NFM_MAX_ORDER + 1];
+        double acc[PMAX + 1];
 #pragma unroll
-        for (int c = 0; c <= NFM_MAX_ORDER; ++c) acc[c] = 0.0;
+        for (int c = 0; c <= PMAX; ++c) acc[c] = 0.0;
         for (uint32_t pb = p0; pb < p1; pb += NFM_TILE) {
             __syncthreads();
             const uint32_t q = pb + threadIdx.x;
             if (threadIdx.x < NFM_TILE && q < p1) {
                 const float *s = A.pos + 3ull * A.perm[q];
                 const double tx = (double)s[0] * A.scale, ty = (double)s[1] * A.scale, tz = (double)s[2] * A.scale;
-                sx[threadIdx.x] = (tx - floor(tx) - 0.5) * A.cellsz;     // offset from the cell centre (reading S5)
-                sy[threadIdx.x] = (ty - floor(ty) - 0.5) * A.cellsz;
-                sz[threadIdx.x] = (tz - floor(tz) - 0.5) * A.cellsz;
-            }
-            __syncthreads();
-            if (nc == 0) continue;
-            const int nt = (int)min((uint32_t)NFM_TILE, p1 - pb);
-            for (int t = 0; t < nt; ++t) {
-                const double X = sx[t], Y = sy[t], Z = sz[t];
-                double m = 1.0;
-                for (int i = 0; i < a; ++i) m = __dmul_rn(m, X);      // mx   = x^a   (mx *= X)
-                for (int i = 0; i < b; ++i) m = __dmul_rn(m, Y);      // mxy  = mx y^b (mxy *= Y)
+                const double X = (tx - floor(tx) - 0.5) * A.cellsz;     // offset from the cell centre (reading S5)
+                const double Y = (ty - floor(ty) - 0.5) * A.cellsz;
+                const double Z = (tz - floor(tz) - 0.5) * A.cellsz;
+                double mx = 1.0, my = 1.0, mz = 1.0;
 #pragma unroll
-                for (int c = 0; c <= NFM_MAX_ORDER; ++c) {
-                    if (c < nc) {
-                        acc[c] = __dadd_rn(acc[c], m);                 // M[a,b,c] += mxyz
-                        m = __dmul_rn(m, Z);                           // mxyz *= Z
+                for (int k = 0; k <= PMAX; ++k) {
+                    if (k <= p) {
+                        xp[threadIdx.x][k] = mx; yp[threadIdx.x][k] = my; zp[threadIdx.x][k] = mz;
+                        mx *= X; my *= Y; mz *= Z;
                     }
                 }
+            }
+            __syncthreads();
+            if (ncw == 0) continue;
+            const int nt = (int)min((uint32_t)NFM_TILE, p1 - pb);
+            for (int t = 0; t < nt; ++t) {
+                const double m = xp[t][a] * yp[t][b];
+#pragma unroll
+                for (int c = 0; c <= PMAX; ++c)
+                    if (c < ncw) acc[c] = fma(m, zp[t][c], acc[c]);       // M[a,b,c] += mxy * Zc[c]
             }
         }
         if (nc > 0) {
             double *o = A.M + (size_t)cell * A.cml + base;
 #pragma unroll
-            for (int c = 0; c <= NFM_MAX_ORDER; ++c)
+            for (int c = 0; c <= PMAX; ++c)
                 if (c < nc) o[c] = acc[c];
         }
     }
@@ -96,7 +111,9 @@ nf_status nf_run_multipoles(nf_ctx *ctx, const float *d_pos, int order, double *
     A.ncell = (int)ctx->ncell; A.order = order; A.cml = (order + 3) * (order + 2) * (order + 1) / 6;
     const int64_t want = ctx->ncell;
     const int grid = (int)(want < (int64_t)ctx->sm_count * 2048 ? want : (int64_t)ctx->sm_count * 2048);
-    k_multipoles<<<grid, nfm_threads(order), 0, st>>>(A); ctx->launches++;
+    if (order <= 8) k_multipoles<8><<<grid, nfm_threads(order), 0, st>>>(A);
+    else k_multipoles<NFM_MAX_ORDER><<<grid, nfm_threads(order), 0, st>>>(A);
+    ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }

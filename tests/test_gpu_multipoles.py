@@ -1,8 +1,10 @@
 """nf_multipoles (Eq. 4) against ``oracle.multipoles`` on the same seeded inputs.
 
-Every element is a double sum of monomials formed by the same multiplications in the same order
-on both sides; the only freedom is whether the host compiler fuses a multiply into the add, so the
-bar is |dM| <= 1e-14 * sum_q |x^a y^b z^c| per element (counts, a = b = c = 0, are exact)."""
+Every element is a double sum of monomials in the same particle order on both sides; the kernel
+forms x^a y^b z^c as (x^a y^b) z^c with the last product fused into the add (the FMA form of
+PAPER.md:199), the oracle by the pseudo-code's running products, so terms differ by a few ulp
+and sums by the rounding of n additions: bar |dM| <= 1e-13 * sum_q |x^a y^b z^c| per element
+(counts, a = b = c = 0, are exact)."""
 import numpy as np
 import pytest
 
@@ -54,7 +56,7 @@ def test_multipoles_match_the_oracle(torch_cuda, NF, oracle_mod, label, cfg, ord
     assert got.shape == ref.shape == (cfg.cpd ** 3, len(idx))
     assert np.array_equal(got[:, 0], ref[:, 0])                              # occupancy: exact
     scale = _abs_moments(pos, cfg.cpd, order, idx)
-    assert np.all(np.abs(got - ref) <= 1e-14 * scale + 1e-300), label
+    assert np.all(np.abs(got - ref) <= 1e-13 * scale + 1e-300), label
 
 
 def test_multipoles_edge_cases(torch_cuda, NF, oracle_mod):
