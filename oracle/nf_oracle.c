@@ -389,3 +389,73 @@ int nfo_multipoles(const float *pos, int64_t N, int cpd, double box, int order, 
     free(cell); free(off);
     return cml;
 }
+
+/*
+ * Kick and Drift of the KDK leapfrog (sec. 3.1 "standard second-order leapfrog
+ * Kick-Drift-Kick"; Table 1: Kick "update velocity from t-1/2 to t+1/2", Drift
+ * "update position from t to t+1"), on float32 state as the paper stores it:
+ *     v <- v + a * dt_kick        x <- x + v_new * dt_drift, wrapped periodically into [0, box)
+ * Readings (K1-K3): each update is evaluated in double from the float32 inputs (one
+ * product, one sum, separately rounded) and rounded to float32 once; the wrap is
+ * w = x - floor(x / box) * box, a result that rounds to box is folded to 0; dt_kick and dt_drift
+ * are plain time intervals (the cosmological drift/kick factors are the caller's).
+ * No fused multiply-add here, so that the CUDA path can reproduce it bit for bit.
+ */
+__attribute__((optimize("fp-contract=off")))
+void nfo_kick_drift(float *pos, float *vel, const float *acc, int64_t N, double dt_kick, double dt_drift, double box) {
+    for (int64_t i = 0; i < 3 * N; ++i) {
+        const double prod = (double)acc[i] * dt_kick;
+        const float v = (float)((double)vel[i] + prod);
+        vel[i] = v;
+        const double step = (double)v * dt_drift;
+        double x = (double)pos[i] + step;
+        const double k = floor(x / box);
+        const double back = k * box;
+        x = x - back;
+        if (x < 0.0) x = 0.0;
+        float xf = (float)x;
+        if (!(xf < (float)box)) xf = 0.0f;
+        pos[i] = xf;
+    }
+}
+
+/*
+ * The particle-dependent part of the time-step criterion, Eq. 1:
+ *     max( min over cells c of [v_rms / a_max]_c ,  v_rms,global / a_max,global )
+ * v_rms = sqrt(mean |v|^2) "computed without subtracting off the mean velocity",
+ * a_max = max |a|, both over the particles of a cell (cells of the CPD^3 grid, binning of nfo_bin)
+ * or of the whole box.  Empty cells and cells with a_max = 0 do not constrain the step.
+ * out[0] = min_c [v_rms/a_max]_c (+inf if no cell constrains), out[1] = v_rms,global / a_max,global,
+ * out[2] = v_rms,global, out[3] = a_max,global.  Returns 0, or -1.
+ */
+int nfo_timestep_ratio(const float *pos, const float *vel, const float *acc, int64_t N, int cpd, double box, double *out) {
+    if (N < 0 || cpd < 1 || !(box > 0)) return -1;
+    const int64_t ncell = (int64_t)cpd * cpd * cpd;
+    int32_t *cell = (int32_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int32_t));
+    double *v2 = (double *)calloc((size_t)ncell, sizeof(double));
+    double *a2 = (double *)calloc((size_t)ncell, sizeof(double));
+    int64_t *cnt = (int64_t *)calloc((size_t)ncell, sizeof(int64_t));
+    if (!cell || !v2 || !a2 || !cnt || nfo_bin(pos, N, cpd, box, cell, NULL) != 0) { free(cell); free(v2); free(a2); free(cnt); return -1; }
+    double gv2 = 0.0, ga2 = 0.0;
+    for (int64_t i = 0; i < N; ++i) {
+        const double vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+        const double ax = acc[3 * i], ay = acc[3 * i + 1], az = acc[3 * i + 2];
+        const double s = vx * vx + vy * vy + vz * vz, t = ax * ax + ay * ay + az * az;
+        v2[cell[i]] += s; cnt[cell[i]]++;
+        if (t > a2[cell[i]]) a2[cell[i]] = t;
+        gv2 += s;
+        if (t > ga2) ga2 = t;
+    }
+    double best = INFINITY;
+    for (int64_t c = 0; c < ncell; ++c) {
+        if (cnt[c] == 0 || a2[c] == 0.0) continue;
+        const double r = sqrt(v2[c] / (double)cnt[c]) / sqrt(a2[c]);
+        if (r < best) best = r;
+    }
+    out[0] = best;
+    out[2] = N > 0 ? sqrt(gv2 / (double)N) : 0.0;
+    out[3] = sqrt(ga2);
+    out[1] = ga2 > 0.0 ? out[2] / out[3] : INFINITY;
+    free(cell); free(v2); free(a2); free(cnt);
+    return 0;
+}

@@ -70,6 +70,10 @@ def _load():
         L.nfo_pair_count.argtypes = [vp, i32, i32]
         L.nfo_accel.restype = i64
         L.nfo_accel.argtypes = [vp, i64, i32, i32, dbl, dbl, dbl, vp, i64, vp, i32]
+        L.nfo_kick_drift.restype = None
+        L.nfo_kick_drift.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl]
+        L.nfo_timestep_ratio.restype = i32
+        L.nfo_timestep_ratio.argtypes = [vp, vp, vp, i64, i32, dbl, vp]
         L.nfo_multipoles.restype = i32
         L.nfo_multipoles.argtypes = [vp, i64, i32, dbl, i32, vp]
         L.nfo_accel_variant.restype = i64
@@ -198,3 +202,24 @@ def multipoles(pos, cpd: int, order: int = 8, box: float = 1.0) -> np.ndarray:
 def multipole_index(order: int):
     """the (a, b, c) triple of every column of ``multipoles`` (the pseudo-code's nesting order)"""
     return [(a, b, c) for a in range(order + 1) for b in range(order - a + 1) for c in range(order - a - b + 1)]
+
+
+def kick_drift(pos, vel, acc, dt_kick: float, dt_drift: float, box: float = 1.0):
+    """Kick then Drift of the KDK leapfrog (Table 1 :379-380) on float32 state.
+    -> (new pos, new vel) float32 [N,3]; the inputs are not modified."""
+    p = _f32pos(pos).copy()
+    v = np.ascontiguousarray(vel, dtype=np.float32).copy()
+    a = np.ascontiguousarray(acc, dtype=np.float32)
+    _load().nfo_kick_drift(p.ctypes.data, v.ctypes.data, a.ctypes.data, p.shape[0], float(dt_kick), float(dt_drift), float(box))
+    return p, v
+
+
+def timestep_ratio(pos, vel, acc, cpd: int, box: float = 1.0) -> np.ndarray:
+    """particle part of Eq. 1: [min_c v_rms/a_max, global v_rms/a_max, v_rms,global, a_max,global]"""
+    p = _f32pos(pos)
+    v = np.ascontiguousarray(vel, dtype=np.float32)
+    a = np.ascontiguousarray(acc, dtype=np.float32)
+    out = np.zeros(4, dtype=np.float64)
+    if _load().nfo_timestep_ratio(p.ctypes.data, v.ctypes.data, a.ctypes.data, p.shape[0], cpd, float(box), out.ctypes.data) != 0:
+        raise ValueError("nfo_timestep_ratio: bad arguments or non-finite position")
+    return out
