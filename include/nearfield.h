@@ -156,6 +156,34 @@ nf_status nf_accel_f64(nf_ctx *ctx, const float *d_pos, int64_t N, double *d_acc
 nf_status nf_multipoles(nf_ctx *ctx, const float *d_pos, int64_t N, int order, double *d_M, void *cuda_stream);
 
 /*
+ * nf_kick_drift -- Kick then Drift of the KDK leapfrog (sec. 3.1; Table 1
+ * PAPER.md:379-380), in place on float32 state:
+ *     v <- v + a * dt_kick ;   x <- x + v_new * dt_drift, wrapped periodically into [0, box).
+ *   d_pos, d_vel [in/out] device, N*3 floats; d_acc [in] device, N*3 floats (e.g. nf_accel's output
+ *   plus the caller's far field).  Each update is evaluated in double (product and sum rounded
+ *   separately) and rounded to float32 once; a wrapped value that rounds to box becomes 0.
+ *   dt_kick / dt_drift are plain intervals (the cosmological kick/drift factors are the caller's);
+ *   a half kick is dt_drift = 0, a pure drift dt_kick = 0.
+ * NF_EINVAL: ctx NULL, N < 0, a NULL buffer with N > 0, a non-finite interval.
+ */
+nf_status nf_kick_drift(nf_ctx *ctx, float *d_pos, float *d_vel, const float *d_acc, int64_t N, double dt_kick, double dt_drift,
+                        void *cuda_stream);
+
+/*
+ * nf_timestep_ratio -- the particle-dependent part of the global time-step criterion, Eq. 1
+ * (PAPER.md:98-102):  max( min over cells of [v_rms / a_max]_c , v_rms,global / a_max,global ), with
+ * v_rms = sqrt(mean |v|^2) (mean velocity not subtracted) and a_max = max |a| over the particles of a
+ * cell of the cpd^3 grid, or of the box.  Empty cells and cells with a_max = 0 do not constrain.
+ *   h_out [out] host, 4 doubles: [0] min_c v_rms/a_max (+inf if none), [1] v_rms,global / a_max,global,
+ *   [2] v_rms,global, [3] a_max,global.  The caller forms
+ *   da = min(eta_H a, eta_acc a H max(h_out[0], h_out[1])).
+ * Runs the binning (A1-A3) of d_pos and one reduction kernel; synchronises the stream.
+ * NF_EINVAL: ctx/h_out NULL, N < 0, a NULL buffer with N > 0.
+ */
+nf_status nf_timestep_ratio(nf_ctx *ctx, const float *d_pos, const float *d_vel, const float *d_acc, int64_t N, double *h_out,
+                            void *cuda_stream);
+
+/*
  * nf_accel_host -- the same through HOST buffers: copies h_pos to the device, runs
  * nf_accel, copies the result back into h_acc and synchronises (this is the end-to-end
  * call bench.py times; pinned host memory makes the copies asynchronous DMA).

@@ -22,7 +22,7 @@ STAGE_NAMES = ["A1_key_hist", "A2_scan", "A3_scatter_rank_gather", "A4_scheduler
 SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", "nf_sync",
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
            "nf_interaction_count", "nf_probe_pipes", "nf_debug_read", "nf_launch_count", "nf_close_radius",
-           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles"]
+           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles", "nf_kick_drift", "nf_timestep_ratio"]
 
 
 class NearFieldError(RuntimeError):
@@ -55,6 +55,10 @@ def load_library() -> ctypes.CDLL:
     L.nf_accel4.argtypes = [vp, vp, i64, vp, vp]
     L.nf_set_softening.restype = i32
     L.nf_set_softening.argtypes = [vp, i32]
+    L.nf_kick_drift.restype = i32
+    L.nf_kick_drift.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, vp]
+    L.nf_timestep_ratio.restype = i32
+    L.nf_timestep_ratio.argtypes = [vp, vp, vp, vp, i64, vp, vp]
     L.nf_multipoles.restype = i32
     L.nf_multipoles.argtypes = [vp, vp, i64, i32, vp, vp]
     L.nf_accel_f64.restype = i32
@@ -214,6 +218,28 @@ class NearField:
         self._check(_L.nf_multipoles(self._h, pos.data_ptr() if N else None, N, int(order), M.data_ptr(),
                                      ctypes.c_void_p(st.cuda_stream)))
         return M
+
+    def kick_drift(self, pos, vel, acc, dt_kick: float, dt_drift: float, stream=None):
+        """nf_kick_drift: in place on CUDA float32 [N,3] tensors pos and vel."""
+        import torch
+        for t in (pos, vel, acc):
+            if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.shape == pos.shape):
+                raise ValueError("pos, vel, acc must be contiguous CUDA float32 tensors of the same shape [N,3]")
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        N = pos.shape[0]
+        self._check(_L.nf_kick_drift(self._h, pos.data_ptr() if N else None, vel.data_ptr() if N else None,
+                                     acc.data_ptr() if N else None, N, float(dt_kick), float(dt_drift), ctypes.c_void_p(st.cuda_stream)))
+
+    def timestep_ratio(self, pos, vel, acc, stream=None) -> np.ndarray:
+        """nf_timestep_ratio -> [min_c v_rms/a_max, global ratio, v_rms,global, a_max,global] (synchronises)."""
+        import torch
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        N = pos.shape[0]
+        self._N = N
+        out = np.zeros(4, dtype=np.float64)
+        self._check(_L.nf_timestep_ratio(self._h, pos.data_ptr() if N else None, vel.data_ptr() if N else None,
+                                         acc.data_ptr() if N else None, N, out.ctypes.data, ctypes.c_void_p(st.cuda_stream)))
+        return out
 
     def accel_ptr(self, d_pos: int, N: int, d_acc: int, cuda_stream: int = 0):
         """raw-pointer form of nf_accel (used by tests of the error paths)."""

@@ -71,7 +71,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     TRY_ALLOC(c->d_col_nblk, (size_t)(c->ncol + 1) * 4);
     TRY_ALLOC(c->d_col_base, (size_t)(c->ncol + 1) * 4);
     TRY_ALLOC(c->d_ctrl, 128 * 4);
-    TRY_ALLOC(c->d_pairs, 16);
+    TRY_ALLOC(c->d_pairs, 64);      // [0..1] pair counter, sink counter; [2..4] time-step reduction (doubles)
     TRY_ALLOC(c->d_nbr, (size_t)4 * 729 * 4);
 #undef TRY_ALLOC
     for (int i = 0; i < 8; ++i)
@@ -246,6 +246,50 @@ extern "C" nf_status nf_multipoles(nf_ctx *c, const float *d_pos, int64_t N, int
     rc = nf_run_binner(c, d_pos, N, st);
     if (rc != NF_OK) return rc;
     return nf_run_multipoles(c, d_pos, order, d_M, st);
+}
+
+extern "C" nf_status nf_kick_drift(nf_ctx *c, float *d_pos, float *d_vel, const float *d_acc, int64_t N, double dt_kick, double dt_drift,
+                                   void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N < 0 || (N > 0 && (!d_pos || !d_vel || !d_acc)) || !isfinite(dt_kick) || !isfinite(dt_drift)) {
+        snprintf(c->err, sizeof c->err, "nf_kick_drift: bad argument (N=%lld)", (long long)N);
+        return NF_EINVAL;
+    }
+    if (N == 0) return NF_OK;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    return nf_run_kick_drift(c, d_pos, d_vel, d_acc, N, dt_kick, dt_drift, (cudaStream_t)cuda_stream);
+}
+
+extern "C" nf_status nf_timestep_ratio(nf_ctx *c, const float *d_pos, const float *d_vel, const float *d_acc, int64_t N, double *h_out,
+                                       void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N < 0 || !h_out || (N > 0 && (!d_pos || !d_vel || !d_acc)) ||
+        (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_timestep_ratio: bad argument (N=%lld)", (long long)N);
+        return NF_EINVAL;
+    }
+    h_out[0] = h_out[1] = INFINITY; h_out[2] = h_out[3] = 0.0;
+    if (N == 0) return NF_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    nf_status rc = ensure_scratch(c, N);
+    if (rc != NF_OK) return rc;
+    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    rc = nf_run_binner(c, d_pos, N, st);
+    if (rc != NF_OK) return rc;
+    double *d3 = (double *)(c->d_pairs + 2);
+    rc = nf_run_timestep_ratio(c, d_vel, d_acc, d3, st);
+    if (rc != NF_OK) return rc;
+    double r[3];
+    NF_CUDA_OK(c, cudaMemcpyAsync(r, d3, sizeof r, cudaMemcpyDeviceToHost, st));
+    NF_CUDA_OK(c, cudaStreamSynchronize(st));
+    h_out[0] = r[0];
+    h_out[2] = sqrt(r[1] / (double)N);
+    h_out[3] = sqrt(r[2]);
+    h_out[1] = r[2] > 0.0 ? h_out[2] / h_out[3] : INFINITY;
+    return NF_OK;
 }
 
 extern "C" nf_status nf_sync(nf_ctx *c) {

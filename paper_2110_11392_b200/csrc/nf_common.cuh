@@ -120,6 +120,9 @@ nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st);
 nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st);
 nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st);
 nf_status nf_run_multipoles(nf_ctx *ctx, const float *d_pos, int order, double *d_M, cudaStream_t st);
+nf_status nf_run_kick_drift(nf_ctx *ctx, float *d_pos, float *d_vel, const float *d_acc, int64_t N, double dt_kick, double dt_drift,
+                            cudaStream_t st);
+nf_status nf_run_timestep_ratio(nf_ctx *ctx, const float *d_vel, const float *d_acc, double *d_out3, cudaStream_t st);
 nf_status nf_run_f64(nf_ctx *ctx, const float *d_pos, int64_t N, double *d_acc, cudaStream_t st);
 nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_interact_setup(nf_ctx *ctx);

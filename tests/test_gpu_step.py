@@ -1,0 +1,103 @@
+"""nf_kick_drift and nf_timestep_ratio (Table 1 :379-380) against the oracle.
+Kick/Drift: bit-exact (both sides evaluate each update in double with separately rounded product
+and sum, and round to float32 once).  Time-step ratio: double sums in a different order: 1e-12."""
+import numpy as np
+import pytest
+
+from paper_2110_11392_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    torch.cuda.set_device(0)
+    return torch
+
+
+@pytest.fixture(scope="module")
+def NF():
+    from paper_2110_11392_b200.binding import NearField
+    return NearField
+
+
+def _state(cfg, seed):
+    rng = np.random.default_rng(seed)
+    pos = W.make_positions(cfg)
+    vel = (rng.normal(size=pos.shape) * 0.3).astype(np.float32)
+    acc = (rng.normal(size=pos.shape) * 5.0).astype(np.float32)
+    return pos, vel, acc
+
+
+@pytest.mark.parametrize("label,cfg", [("cfg1", W.CONFIGS[1]), ("cfg3 @cpd10", W.scaled(W.CONFIGS[3], 10)), ("cfg2 full", W.CONFIGS[2])])
+@pytest.mark.parametrize("dtk,dtd", [(0.01, 0.02), (0.005, 0.0), (0.0, 0.7), (-0.01, -0.02)])
+def test_kick_drift_bit_exact(torch_cuda, NF, oracle_mod, label, cfg, dtk, dtd):
+    pos, vel, acc = _state(cfg, 1)
+    rp, rv = oracle_mod.kick_drift(pos, vel, acc, dtk, dtd)
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        dp, dv, da = (torch_cuda.from_numpy(x.copy()).cuda() for x in (pos, vel, acc))
+        nf.kick_drift(dp, dv, da, dtk, dtd)
+        torch_cuda.cuda.synchronize()
+        gp, gv = dp.cpu().numpy(), dv.cpu().numpy()
+    assert np.array_equal(gv, rv)
+    assert np.array_equal(gp, rp)
+    assert np.all((gp >= 0) & (gp < 1))
+
+
+def test_kick_drift_other_box_and_empty(torch_cuda, NF, oracle_mod):
+    rng = np.random.default_rng(2)
+    pos = (rng.random((5000, 3)) * 5).astype(np.float32)
+    vel = rng.normal(size=pos.shape).astype(np.float32) * 3
+    acc = rng.normal(size=pos.shape).astype(np.float32)
+    rp, rv = oracle_mod.kick_drift(pos, vel, acc, 0.1, 2.0, box=5.0)
+    with NF(7, 2, 1e-3, 5.0) as nf:
+        dp, dv, da = (torch_cuda.from_numpy(x.copy()).cuda() for x in (pos, vel, acc))
+        nf.kick_drift(dp, dv, da, 0.1, 2.0)
+        e = torch_cuda.zeros((0, 3), dtype=torch_cuda.float32, device="cuda")
+        nf.kick_drift(e, e, e, 0.1, 0.1)
+        torch_cuda.cuda.synchronize()
+        assert np.array_equal(dp.cpu().numpy(), rp) and np.array_equal(dv.cpu().numpy(), rv)
+        assert float(dp.max()) < 5.0 and float(dp.min()) >= 0.0
+
+
+@pytest.mark.parametrize("label,cfg", [("cfg1", W.CONFIGS[1]), ("cfg3 @cpd10", W.scaled(W.CONFIGS[3], 10)), ("cfg5 @cpd9", W.scaled(W.CONFIGS[5], 9))])
+def test_timestep_ratio(torch_cuda, NF, oracle_mod, label, cfg):
+    pos, vel, acc = _state(cfg, 3)
+    cell, _ = oracle_mod.bin_particles(pos, cfg.cpd)
+    acc[cell == cell[0]] = 0                              # one cell without acceleration: must not constrain
+    ref = oracle_mod.timestep_ratio(pos, vel, acc, cfg.cpd)
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        got = nf.timestep_ratio(*(torch_cuda.from_numpy(x).cuda() for x in (pos, vel, acc)))
+        none = nf.timestep_ratio(torch_cuda.from_numpy(pos).cuda(), torch_cuda.from_numpy(vel).cuda(),
+                                 torch_cuda.zeros_like(torch_cuda.from_numpy(acc)).cuda())
+    assert np.allclose(got, ref, rtol=1e-12, atol=0), (got, ref)
+    assert got[3] == ref[3]                               # a maximum: exact
+    assert np.isinf(none[0]) and np.isinf(none[1]) and none[3] == 0.0
+
+
+def test_leapfrog_step_with_the_near_field(torch_cuda, NF, oracle_mod):
+    """one KDK step driven by nf_accel on the GPU against the same step driven by the oracle's
+    accelerations: positions agree to float32 rounding of a 1e-5-accurate acceleration."""
+    cfg = W.scaled(W.CONFIGS[2], 9)
+    pos = W.make_positions(cfg)
+    vel = np.zeros_like(pos)
+    dt = 1e-3
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        dp, dv = torch_cuda.from_numpy(pos.copy()).cuda(), torch_cuda.from_numpy(vel.copy()).cuda()
+        a0 = nf.accel(dp)
+        nf.kick_drift(dp, dv, a0, dt / 2, dt)
+        a1 = nf.accel(dp)
+        nf.kick_drift(dp, dv, a1, dt / 2, 0.0)
+        nf.sync()
+        gp, gv = dp.cpu().numpy(), dv.cpu().numpy()
+    r0, _ = oracle_mod.accel(pos, cfg.cpd, cfg.R, cfg.eps_p)
+    p1, v1 = oracle_mod.kick_drift(pos, vel, r0.astype(np.float32), dt / 2, dt)
+    r1, _ = oracle_mod.accel(p1, cfg.cpd, cfg.R, cfg.eps_p)
+    _, v2 = oracle_mod.kick_drift(p1, v1, r1.astype(np.float32), dt / 2, 0.0)
+    d = np.abs(gp.astype(np.float64) - p1)
+    d = np.minimum(d, 1 - d)
+    assert d.max() <= 2e-7
+    vr = np.sqrt((v2.astype(np.float64) ** 2).sum(1).mean())
+    assert np.abs(gv - v2).max() <= 2e-5 * vr
