@@ -41,13 +41,11 @@
 #ifndef NF_CELL_PAD
 #define NF_CELL_PAD 4             // every cell is padded to a multiple of this many slots (power of two, >= 2)
 #endif
-#ifndef NF_UNROLL
-#endif
 #ifndef NF_MIN_CTAS
 #define NF_MIN_CTAS 4             // resident CTAs per SM the interaction kernel is compiled for
 #endif
 #ifndef NF_PRODUCER_SLEEP_NS
-#define NF_PRODUCER_SLEEP_NS 0    // back-off of the producer warp while its ring slot is still in use
+#define NF_PRODUCER_SLEEP_NS 0    // back-off of a dedicated producer warp (NF_PRODUCER_WARP = 1) while its ring slot is in use
 #endif
 #ifndef NF_CONSUMER_SLEEP_NS
 #define NF_CONSUMER_SLEEP_NS 0

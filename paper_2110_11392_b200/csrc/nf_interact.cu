@@ -1,22 +1,25 @@
 // nf_interact.cu -- steps A4..A6: pencil scheduler, pencil-on-pencil interaction kernel with
 // fused un-permute, plus the neighbour-list and pair-count exports.
 //
-// Paper basis: PAPER.md:226-236 (sec. 3.4.2 pencil-on-pencil; sink blocks; one sink per
-// thread in registers, sources staged in shared memory), PAPER.md:132 (Eq. 3)
-// (hand-off to 1/r^2 "with a min instead of a conditional").  What differs from the paper's
-// V100 design, and why, is in DESIGN.md "Kernel design":
+// Paper basis: PAPER.md:226-236 (sec. 3.4.2 pencil-on-pencil; sink blocks; sinks in registers,
+// sources staged in shared memory), PAPER.md:132 (Eq. 3), PAPER.md:254 (hand-off to 1/r^2 "with
+// a min instead of a conditional").  What differs from the paper's V100 design, and why, is in
+// DESIGN.md sections 6-8:
 //   * sinks AND sources are z-pencils (z is the fastest cell index, so the source cells
 //     (i+a, j+b, k-R..k+R) of one (a,b) column are ONE contiguous range of the sorted planes
-//     -> one cp.async.bulk per coordinate plane per column, completed on an mbarrier);
-//   * 32 consecutive grid-order sinks per warp regardless of cell boundaries; a lane whose
-//     cell is more than R cells from the current source cell is masked by moving its sink to
-//     -NF_BIG, which makes its contribution exactly 0 (no per-interaction predicate);
-//   * two sources per thread-iteration in packed fma.rn.f32x2 / add.f32x2 / mul.f32x2, so the
-//     FMA pipe (2 cycles per packed warp-instruction) is the bound, not the issue slots;
+//     -> one cp.async.bulk per coordinate plane per column window, completed on an mbarrier);
+//   * 64 consecutive grid-order sinks per warp (two per thread, same cell) regardless of cell
+//     boundaries; source cells c and c+2R+1, each needed by only part of the warp, are read in
+//     the same pass by disjoint lane groups; a lane that needs neither is masked by moving its
+//     sink to -NF_BIG, which makes its contribution exactly 0 (no per-interaction predicate);
+//   * four sources per LDS.128 and plane, shared by the thread's two sinks; two sources per
+//     packed fma.rn.f32x2 / add.f32x2 / mul.f32x2, so the FMA pipe is the bound, not the issue
+//     slots or the LSU;
 //   * source cells that cannot hold r < eps_s skip the spline (11 instead of 14 FMA-pipe ops);
-//   * a dedicated producer warp streams (column, z-run, chunk) segments through an
-//     NF_NSTAGE-deep full/empty mbarrier ring; persistent CTAs pull sink blocks from an
-//     atomic counter in heavy-first order;
+//     with a close-pair radius the near cells clamp r^-3 and close_scan repairs close pairs in double;
+//   * no producer warp: consumer warp 0 refills the NF_NSTAGE-deep full/empty mbarrier ring of
+//     (column, z-run, chunk) stages from a cursor in shared memory; persistent CTAs pull sink
+//     blocks from an atomic counter in grid order;
 //   * A6 is fused: each thread writes gm/cell^2 * a straight to d_acc[perm[slot]].
 #include "nf_common.cuh"
 
