@@ -318,3 +318,37 @@ def test_full_size_configs_sampled(torch_cuda, NF, oracle_mod, k, n_random, n_ex
     # property that holds at any size: total momentum ~ 0
     s = got.astype(np.float64)
     assert np.abs(s.sum(0)).max() <= 1e-5 * np.abs(s).sum()
+
+
+# ----------------------------------------------------------------------------- other radii and occupancies
+# The pair loop processes source cells c and c + 2R+1 in one pass (disjoint lane groups); these
+# cases move the pairing distance (R = 1, 3, 4), make a warp's 64 sinks span many cells (2 per
+# cell: windows longer than 2(2R+1) cells, several pairing blocks) or a fraction of one cell.
+RADII = [
+    ("R1 uniform 40/cell cpd8", W.Config("r1u", 8, 1, 40 * 8 ** 3, "uniform", 1.0 / (40 * 8 ** 3) ** (1 / 3) / 40, seed=5)),
+    ("R1 clustered cpd9", W.Config("r1p", 9, 1, 64 * 9 ** 3, "plummer", 1.0 / (64 * 9 ** 3) ** (1 / 3) / 40, seed=6, n_spheres=60)),
+    ("R4 uniform 20/cell cpd10", W.Config("r4u", 10, 4, 20 * 10 ** 3, "uniform", 1.0 / (20 * 10 ** 3) ** (1 / 3) / 40, seed=7)),
+    ("R4 = (cpd-1)/2 cpd9", W.Config("r4w", 9, 4, 30 * 9 ** 3, "uniform", 1.0 / (30 * 9 ** 3) ** (1 / 3) / 40, seed=8)),
+    ("R2 sparse 2/cell cpd16", W.Config("r2s", 16, 2, 2 * 16 ** 3, "uniform", 1.0 / (2 * 16 ** 3) ** (1 / 3) / 40, seed=9)),
+    ("R3 sparse 3/cell cpd12", W.Config("r3s", 12, 3, 3 * 12 ** 3, "uniform", 1.0 / (3 * 12 ** 3) ** (1 / 3) / 40, seed=10)),
+    ("R2 dense 600/cell cpd5", W.Config("r2d", 5, 2, 600 * 5 ** 3, "uniform", 1.0 / (600 * 5 ** 3) ** (1 / 3) / 40, seed=11)),
+]
+
+
+@pytest.mark.parametrize("label,cfg", RADII, ids=[r[0] for r in RADII])
+def test_other_radii_and_occupancies_elementwise(torch_cuda, NF, oracle_mod, label, cfg):
+    pos = W.make_positions(cfg)
+    got, pairs, _ = gpu_accel(torch_cuda, NF, pos, cfg.cpd, cfg.R, cfg.eps_p)
+    ref, ref_pairs = oracle_mod.accel(pos, cfg.cpd, cfg.R, cfg.eps_p)
+    assert pairs == ref_pairs
+    check(got, ref, label=label)
+    # and with the close-pair path forced off / forced wide: both regimes of the kernel
+    for rc in (0.0, 0.2):
+        alt, _, _ = gpu_accel(torch_cuda, NF, pos, cfg.cpd, cfg.R, cfg.eps_p, opts={"rc_cells": rc})
+        d = np.linalg.norm(alt - ref, axis=1)
+        rms = np.sqrt((ref ** 2).sum(1).mean())
+        assert np.isfinite(alt).all()
+        if rc > 0:
+            assert d.max() <= TOL_ABS * rms, f"{label} rc={rc}: {d.max() / rms:.3e}"
+        else:
+            assert np.median(d / np.maximum(np.linalg.norm(ref, axis=1), 1e-300)) <= 1e-5      # float32 min form: looser, still sane
