@@ -459,3 +459,42 @@ int nfo_timestep_ratio(const float *pos, const float *vel, const float *acc, int
     free(cell); free(v2); free(a2); free(cnt);
     return 0;
 }
+
+/*
+ * Taylor evaluation of the far field ("evaluating the force from the resulting Taylor
+ * series of the potential in every cell"; "the output is a 3-vector of acceleration for
+ * every particle ... about 3 times more floating-point work").  The paper does not print the
+ * series; reading (F1): the cell's Taylors are the coefficients T^{a,b,c} of the potential
+ * in the same complete basis and index order as the multipoles,
+ *     phi(x,y,z) = sum_{a+b+c <= p} T^{a,b,c} x^a y^b z^c,   (x,y,z) = offset from the cell centre,
+ * (any factorials are folded into T by whoever produces it), and the far-field acceleration is
+ *     a = -grad phi = -( sum a T x^(a-1) y^b z^c,  sum b T x^a y^(b-1) z^c,  sum c T x^a y^b z^(c-1) ).
+ * T: ncell * cml doubles, cell-major.  acc[N][3] double, input order.  Returns 0, or -1.
+ */
+int nfo_taylor_accel(const float *pos, int64_t N, int cpd, double box, int order, const double *T, double *acc) {
+    if (N < 0 || cpd < 1 || !(box > 0) || order < 0 || order > 16) return -1;
+    const int cml = (order + 3) * (order + 2) * (order + 1) / 6;
+    int32_t *cell = (int32_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int32_t));
+    double *off = (double *)malloc((size_t)(N > 0 ? N : 1) * 3 * sizeof(double));
+    if (!cell || !off || nfo_bin(pos, N, cpd, box, cell, off) != 0) { free(cell); free(off); return -1; }
+    for (int64_t q = 0; q < N; ++q) {
+        const double *Tc = T + (size_t)cell[q] * cml;
+        const double X = off[3 * q], Y = off[3 * q + 1], Z = off[3 * q + 2];
+        double xp[18], yp[18], zp[18];
+        xp[0] = yp[0] = zp[0] = 1.0;
+        for (int k = 1; k <= order; ++k) { xp[k] = xp[k - 1] * X; yp[k] = yp[k - 1] * Y; zp[k] = zp[k - 1] * Z; }
+        double gx = 0.0, gy = 0.0, gz = 0.0;
+        int idx = 0;
+        for (int a = 0; a <= order; ++a)
+            for (int b = 0; b <= order - a; ++b)
+                for (int c = 0; c <= order - a - b; ++c, ++idx) {
+                    const double t = Tc[idx];
+                    if (a > 0) gx += t * a * xp[a - 1] * yp[b] * zp[c];
+                    if (b > 0) gy += t * b * xp[a] * yp[b - 1] * zp[c];
+                    if (c > 0) gz += t * c * xp[a] * yp[b] * zp[c - 1];
+                }
+        acc[3 * q] = -gx; acc[3 * q + 1] = -gy; acc[3 * q + 2] = -gz;
+    }
+    free(cell); free(off);
+    return 0;
+}

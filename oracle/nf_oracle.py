@@ -74,6 +74,8 @@ def _load():
         L.nfo_kick_drift.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl]
         L.nfo_timestep_ratio.restype = i32
         L.nfo_timestep_ratio.argtypes = [vp, vp, vp, i64, i32, dbl, vp]
+        L.nfo_taylor_accel.restype = i32
+        L.nfo_taylor_accel.argtypes = [vp, i64, i32, dbl, i32, vp, vp]
         L.nfo_multipoles.restype = i32
         L.nfo_multipoles.argtypes = [vp, i64, i32, dbl, i32, vp]
         L.nfo_accel_variant.restype = i64
@@ -223,3 +225,17 @@ def timestep_ratio(pos, vel, acc, cpd: int, box: float = 1.0) -> np.ndarray:
     if _load().nfo_timestep_ratio(p.ctypes.data, v.ctypes.data, a.ctypes.data, p.shape[0], cpd, float(box), out.ctypes.data) != 0:
         raise ValueError("nfo_timestep_ratio: bad arguments or non-finite position")
     return out
+
+
+def taylor_accel(pos, T, cpd: int, order: int = 8, box: float = 1.0) -> np.ndarray:
+    """Far-field acceleration -grad phi from per-cell Taylor coefficients of the potential in the
+    complete basis (reading F1).  T: [cpd^3, cml] float64 -> acc float64 [N,3]."""
+    p = _f32pos(pos)
+    cml = (order + 3) * (order + 2) * (order + 1) // 6
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    if T.shape != (cpd ** 3, cml):
+        raise ValueError(f"T must have shape {(cpd ** 3, cml)}")
+    acc = np.zeros((p.shape[0], 3), dtype=np.float64)
+    if _load().nfo_taylor_accel(p.ctypes.data, p.shape[0], cpd, float(box), int(order), T.ctypes.data, acc.ctypes.data) != 0:
+        raise ValueError("nfo_taylor_accel: bad arguments or non-finite position")
+    return acc
