@@ -156,6 +156,22 @@ nf_status nf_accel_f64(nf_ctx *ctx, const float *d_pos, int64_t N, double *d_acc
 nf_status nf_multipoles(nf_ctx *ctx, const float *d_pos, int64_t N, int order, double *d_M, void *cuda_stream);
 
 /*
+ * nf_taylor_accel -- far-field acceleration of every particle from its cell's Taylor series of
+ * the potential (TaylorForce, Table 1).  The paper does not print
+ * the series; this library's reading: d_T holds, per cell, the coefficients T^{a,b,c} of
+ *     phi(x,y,z) = sum_{a+b+c <= order} T^{a,b,c} x^a y^b z^c,  (x,y,z) = offset from the cell centre,
+ * in the complete basis and element order of nf_multipoles (factorials folded into T), and
+ *     a = -grad phi.
+ *   d_T   [in]  device, cpd^3 * cml doubles, cell-major;  d_acc [out] device, N*3 floats, input
+ *   order: written, or added to when accumulate != 0 (e.g. onto nf_accel's near field).
+ * Evaluated in double, rounded to float32 once.  Runs the binning (A1-A3) and one kernel.  Producing
+ * T (reduced basis, FFTs, derivatives-tensor convolution) is not part of this library.
+ * NF_EINVAL: ctx NULL, N < 0, a NULL buffer with N > 0, order outside [0, NF_MAX_MULTIPOLE_ORDER].
+ */
+nf_status nf_taylor_accel(nf_ctx *ctx, const float *d_pos, int64_t N, int order, const double *d_T, float *d_acc, int accumulate,
+                          void *cuda_stream);
+
+/*
  * nf_kick_drift -- Kick then Drift of the KDK leapfrog (sec. 3.1; Table 1
  * PAPER.md:379-380), in place on float32 state:
  *     v <- v + a * dt_kick ;   x <- x + v_new * dt_drift, wrapped periodically into [0, box).

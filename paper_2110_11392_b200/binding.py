@@ -22,7 +22,7 @@ STAGE_NAMES = ["A1_key_hist", "A2_scan", "A3_scatter_rank_gather", "A4_scheduler
 SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", "nf_sync",
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
            "nf_interaction_count", "nf_probe_pipes", "nf_debug_read", "nf_launch_count", "nf_close_radius",
-           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles", "nf_kick_drift", "nf_timestep_ratio"]
+           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles", "nf_kick_drift", "nf_timestep_ratio", "nf_taylor_accel"]
 
 
 class NearFieldError(RuntimeError):
@@ -59,6 +59,8 @@ def load_library() -> ctypes.CDLL:
     L.nf_kick_drift.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, vp]
     L.nf_timestep_ratio.restype = i32
     L.nf_timestep_ratio.argtypes = [vp, vp, vp, vp, i64, vp, vp]
+    L.nf_taylor_accel.restype = i32
+    L.nf_taylor_accel.argtypes = [vp, vp, i64, i32, vp, vp, i32, vp]
     L.nf_multipoles.restype = i32
     L.nf_multipoles.argtypes = [vp, vp, i64, i32, vp, vp]
     L.nf_accel_f64.restype = i32
@@ -218,6 +220,21 @@ class NearField:
         self._check(_L.nf_multipoles(self._h, pos.data_ptr() if N else None, N, int(order), M.data_ptr(),
                                      ctypes.c_void_p(st.cuda_stream)))
         return M
+
+    def taylor_accel(self, pos, T, order: int = 8, acc=None, accumulate: bool = False, stream=None):
+        """nf_taylor_accel: T float64 [cpd^3, cml] on the device -> acc float32 [N,3] (written or added to)."""
+        import torch
+        N = pos.shape[0]
+        cml = (order + 3) * (order + 2) * (order + 1) // 6
+        if not (T.is_cuda and T.dtype == torch.float64 and T.is_contiguous() and tuple(T.shape) == (self.cpd ** 3, cml)):
+            raise ValueError(f"T must be a contiguous CUDA float64 tensor of shape {(self.cpd ** 3, cml)}")
+        if acc is None:
+            acc = torch.zeros_like(pos)
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        self._N = N
+        self._check(_L.nf_taylor_accel(self._h, pos.data_ptr() if N else None, N, int(order), T.data_ptr(),
+                                       acc.data_ptr() if N else None, 1 if accumulate else 0, ctypes.c_void_p(st.cuda_stream)))
+        return acc
 
     def kick_drift(self, pos, vel, acc, dt_kick: float, dt_drift: float, stream=None):
         """nf_kick_drift: in place on CUDA float32 [N,3] tensors pos and vel."""

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnearfield_b200.so")
-SOURCES = ["nf_api.cu", "nf_binner.cu", "nf_interact.cu", "nf_f64.cu", "nf_multipoles.cu", "nf_step.cu", "nf_probe.cu"]
+SOURCES = ["nf_api.cu", "nf_binner.cu", "nf_interact.cu", "nf_f64.cu", "nf_multipoles.cu", "nf_taylor.cu", "nf_step.cu", "nf_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xcompiler", "-Wno-format-truncation"]
 

@@ -292,6 +292,26 @@ extern "C" nf_status nf_timestep_ratio(nf_ctx *c, const float *d_pos, const floa
     return NF_OK;
 }
 
+extern "C" nf_status nf_taylor_accel(nf_ctx *c, const float *d_pos, int64_t N, int order, const double *d_T, float *d_acc, int accumulate,
+                                     void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N < 0 || (N > 0 && (!d_pos || !d_T || !d_acc)) || order < 0 || order > NF_MAX_MULTIPOLE_ORDER ||
+        (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_taylor_accel: bad argument (N=%lld order=%d)", (long long)N, order);
+        return NF_EINVAL;
+    }
+    if (N == 0) return NF_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    nf_status rc = ensure_scratch(c, N);
+    if (rc != NF_OK) return rc;
+    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    rc = nf_run_binner(c, d_pos, N, st);
+    if (rc != NF_OK) return rc;
+    return nf_run_taylor(c, d_pos, order, d_T, d_acc, accumulate ? 1 : 0, st);
+}
+
 extern "C" nf_status nf_sync(nf_ctx *c) {
     if (!c) return NF_EINVAL;
     if (!c->have_last) return NF_OK;

@@ -121,6 +121,7 @@ nf_status nf_run_multipoles(nf_ctx *ctx, const float *d_pos, int order, double *
 nf_status nf_run_kick_drift(nf_ctx *ctx, float *d_pos, float *d_vel, const float *d_acc, int64_t N, double dt_kick, double dt_drift,
                             cudaStream_t st);
 nf_status nf_run_timestep_ratio(nf_ctx *ctx, const float *d_vel, const float *d_acc, double *d_out3, cudaStream_t st);
+nf_status nf_run_taylor(nf_ctx *ctx, const float *d_pos, int order, const double *d_T, float *d_acc, int accumulate, cudaStream_t st);
 nf_status nf_run_f64(nf_ctx *ctx, const float *d_pos, int64_t N, double *d_acc, cudaStream_t st);
 nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_interact_setup(nf_ctx *ctx);

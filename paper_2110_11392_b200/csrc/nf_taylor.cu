@@ -1,0 +1,90 @@
+// nf_taylor.cu -- nf_taylor_accel: the far-field acceleration of every particle from its cell's
+// Taylor series of the potential, the step before NearForce in the paper's
+// pipeline (TaylorForce, Table 1).  Reading F1: coefficients T^{a,b,c} of
+//     phi(x,y,z) = sum_{a+b+c <= p} T^{a,b,c} x^a y^b z^c,   (x,y,z) = offset from the cell centre,
+// in the complete basis and index order of nf_multipoles;  a = -grad phi.
+//
+// Mapping: one CTA of 64 threads per cell; the cell's cml coefficients are staged once in shared
+// memory (all threads then read the same coefficient: broadcast), one particle per thread (more
+// in turn for fuller cells) with its power tables x^k, y^k, z^k in registers, in double.  Per
+// (a, b) the z-polynomial and its derivative come from one Horner pass over c; the sums over b and
+// a use the power tables.  About 4 FMA per coefficient: FP64-pipe bound, 3.2 GB of coefficients
+// read once at config 4.  The result is rounded to float32 once and written (or added) in input order.
+#include "nf_common.cuh"
+
+#define NFT_THREADS 64
+
+struct TaylorArgs {
+    const float *pos;
+    const uint32_t *offsets, *perm;
+    const double *T;
+    float *acc;
+    double scale, cellsz;
+    int ncell, order, cml, accumulate;
+};
+
+template <int PMAX>
+__global__ void __launch_bounds__(NFT_THREADS) k_taylor(const TaylorArgs A) {
+    extern __shared__ double sT[];
+    const int p = A.order;
+    for (int cell = blockIdx.x; cell < A.ncell; cell += gridDim.x) {
+        const uint32_t p0 = A.offsets[cell], p1 = A.offsets[cell + 1];
+        if (p0 == p1) continue;
+        __syncthreads();
+        for (int i = threadIdx.x; i < A.cml; i += NFT_THREADS) sT[i] = A.T[(size_t)cell * A.cml + i];
+        __syncthreads();
+        for (uint32_t q = p0 + threadIdx.x; q < p1; q += NFT_THREADS) {
+            const uint32_t pi = A.perm[q];
+            const float *s = A.pos + 3ull * pi;
+            const double tx = (double)s[0] * A.scale, ty = (double)s[1] * A.scale, tz = (double)s[2] * A.scale;
+            const double X = (tx - floor(tx) - 0.5) * A.cellsz, Y = (ty - floor(ty) - 0.5) * A.cellsz, Z = (tz - floor(tz) - 0.5) * A.cellsz;
+            double xp[PMAX + 1], yp[PMAX + 1];
+            xp[0] = 1.0; yp[0] = 1.0;
+#pragma unroll
+            for (int k = 1; k <= PMAX; ++k) { xp[k] = xp[k - 1] * X; yp[k] = yp[k - 1] * Y; }
+            double gx = 0.0, gy = 0.0, gz = 0.0;
+            int idx = 0;
+#pragma unroll
+            for (int a = 0; a <= PMAX; ++a) {
+                if (a > p) break;
+                double s0 = 0.0, s1 = 0.0, sq = 0.0;      // sum_b P y^b, sum_b b P y^(b-1), sum_b Q y^b
+#pragma unroll
+                for (int b = 0; b <= PMAX - a; ++b) {
+                    if (b > p - a) break;
+                    const int nc = p - a - b + 1;
+                    // Horner over c from the top: P = sum_c T z^c, Q = dP/dz
+                    double P = 0.0, Q = 0.0;
+                    for (int c = nc - 1; c >= 0; --c) {
+                        Q = fma(Q, Z, P);
+                        P = fma(P, Z, sT[idx + c]);
+                    }
+                    idx += nc;
+                    s0 = fma(P, yp[b], s0);
+                    if (b > 0) s1 = fma(P * (double)b, yp[b - 1], s1);
+                    sq = fma(Q, yp[b], sq);
+                }
+                if (a > 0) gx = fma(s0 * (double)a, xp[a - 1], gx);
+                gy = fma(s1, xp[a], gy);
+                gz = fma(sq, xp[a], gz);
+            }
+            float *o = A.acc + 3ull * pi;
+            if (A.accumulate) { o[0] += (float)(-gx); o[1] += (float)(-gy); o[2] += (float)(-gz); }
+            else { o[0] = (float)(-gx); o[1] = (float)(-gy); o[2] = (float)(-gz); }
+        }
+    }
+}
+
+nf_status nf_run_taylor(nf_ctx *ctx, const float *d_pos, int order, const double *d_T, float *d_acc, int accumulate, cudaStream_t st) {
+    TaylorArgs A;
+    A.pos = d_pos; A.offsets = ctx->d_offsets; A.perm = ctx->d_perm_true; A.T = d_T; A.acc = d_acc;
+    A.scale = ctx->prm.scale; A.cellsz = ctx->box / (double)ctx->cpd;
+    A.ncell = (int)ctx->ncell; A.order = order; A.cml = (order + 3) * (order + 2) * (order + 1) / 6; A.accumulate = accumulate;
+    const int64_t want = ctx->ncell;
+    const int grid = (int)(want < (int64_t)ctx->sm_count * 2048 ? want : (int64_t)ctx->sm_count * 2048);
+    const size_t smem = (size_t)A.cml * sizeof(double);
+    if (order <= 8) k_taylor<8><<<grid, NFT_THREADS, smem, st>>>(A);
+    else k_taylor<NF_MAX_MULTIPOLE_ORDER><<<grid, NFT_THREADS, smem, st>>>(A);
+    ctx->launches++;
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
