@@ -38,7 +38,9 @@ struct MultipoleArgs {
 // PMAX = compile-time bound of the order (8: the paper's choice; NFM_MAX_ORDER: any order)
 template <int PMAX>
 __global__ void __launch_bounds__(160) k_multipoles(const MultipoleArgs A) {
-    __shared__ double xp[NFM_TILE][PMAX + 1], yp[NFM_TILE][PMAX + 1], zp[NFM_TILE][PMAX + 1];
+    constexpr int ZROW = (PMAX + 2) & ~1;       // z-power rows padded to an even length: read as double2 (LDS.128 broadcasts)
+    __shared__ double xp[NFM_TILE][PMAX + 1], yp[NFM_TILE][PMAX + 1];
+    __shared__ __align__(16) double zp[NFM_TILE][ZROW];
     const int p = A.order;
     // thread t -> the t-th (a, b) pair in order of descending element count nc = p - a - b + 1
     // (ties in basis order), and the index of the pair's first element in the basis order
@@ -84,15 +86,24 @@ __global__ void __launch_bounds__(160) k_multipoles(const MultipoleArgs A) {
                         mx *= X; my *= Y; mz *= Z;
                     }
                 }
+#pragma unroll
+                for (int k = 0; k < ZROW; ++k)
+                    if (k > p) zp[threadIdx.x][k] = 0.0;           // unused powers read as 0: the extra FMA of a pair adds nothing
             }
             __syncthreads();
             if (ncw == 0) continue;
             const int nt = (int)min((uint32_t)NFM_TILE, p1 - pb);
             for (int t = 0; t < nt; ++t) {
                 const double m = xp[t][a] * yp[t][b];
+                const double2 *zr = reinterpret_cast<const double2 *>(zp[t]);
 #pragma unroll
-                for (int c = 0; c <= PMAX; ++c)
-                    if (c < ncw) acc[c] = fma(m, zp[t][c], acc[c]);       // M[a,b,c] += mxy * Zc[c]
+                for (int c = 0; c <= PMAX; c += 2) {
+                    if (c < ncw) {
+                        const double2 zz = zr[c >> 1];
+                        acc[c] = fma(m, zz.x, acc[c]);                      // M[a,b,c] += mxy * Zc[c]
+                        if (c + 1 <= PMAX) acc[c + 1 <= PMAX ? c + 1 : c] = fma(m, zz.y, acc[c + 1 <= PMAX ? c + 1 : c]);
+                    }
+                }
             }
         }
         if (nc > 0) {
