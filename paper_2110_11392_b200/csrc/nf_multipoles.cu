@@ -20,6 +20,7 @@
 // memory -- the FMA form the paper itself proposes ("M[a,b,c] += mxy*Zc[c]").
 // Particles are added in ascending grid order.  Bound: FP64 pipe (cml FMAs + (p+1)(p+2)/2
 // multiplies + 3p table multiplies per 12-byte particle, against 3.2 GB of output at config 4).
+#include <type_traits>
 #include "nf_common.cuh"
 
 #define NFM_TILE 32
@@ -93,18 +94,27 @@ __global__ void __launch_bounds__(160) k_multipoles(const MultipoleArgs A) {
             __syncthreads();
             if (ncw == 0) continue;
             const int nt = (int)min((uint32_t)NFM_TILE, p1 - pb);
-            for (int t = 0; t < nt; ++t) {
-                const double m = xp[t][a] * yp[t][b];
-                const double2 *zr = reinterpret_cast<const double2 *>(zp[t]);
+            // the loop over the tile's particles, with the warp's element bound NCW as a compile-time
+            // constant where it is known (p = 8: 9 for the first warp, 2 for the second): no predicates
+            auto tile = [&](auto ncw_tag) {
+                constexpr int NCW = decltype(ncw_tag)::value;
+                const double *xr = &xp[0][a], *yr = &yp[0][b];
+                for (int t = 0; t < nt; ++t) {
+                    const double m = xr[t * (PMAX + 1)] * yr[t * (PMAX + 1)];
+                    const double2 *zr = reinterpret_cast<const double2 *>(zp[t]);
 #pragma unroll
-                for (int c = 0; c <= PMAX; c += 2) {
-                    if (c < ncw) {
-                        const double2 zz = zr[c >> 1];
-                        acc[c] = fma(m, zz.x, acc[c]);                      // M[a,b,c] += mxy * Zc[c]
-                        if (c + 1 <= PMAX) acc[c + 1 <= PMAX ? c + 1 : c] = fma(m, zz.y, acc[c + 1 <= PMAX ? c + 1 : c]);
+                    for (int c = 0; c < (NCW > 0 ? NCW : PMAX + 1); c += 2) {
+                        if (NCW > 0 || c < ncw) {
+                            const double2 zz = zr[c >> 1];
+                            acc[c] = fma(m, zz.x, acc[c]);                      // M[a,b,c] += mxy * Zc[c]
+                            if (c + 1 <= PMAX) acc[c + 1 <= PMAX ? c + 1 : c] = fma(m, zz.y, acc[c + 1 <= PMAX ? c + 1 : c]);
+                        }
                     }
                 }
-            }
+            };
+            if (PMAX == 8 && ncw == 9) tile(std::integral_constant<int, 9>{});
+            else if (PMAX == 8 && ncw == 2) tile(std::integral_constant<int, 2>{});
+            else tile(std::integral_constant<int, 0>{});
         }
         if (nc > 0) {
             double *o = A.M + (size_t)cell * A.cml + base;
