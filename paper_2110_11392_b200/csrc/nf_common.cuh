@@ -23,6 +23,12 @@
 #ifndef NF_PRODUCER_WARP
 #define NF_PRODUCER_WARP 0        // 1: a dedicated producer warp per CTA; 0: consumer warp 0 also fills the ring
 #endif
+#ifndef NF_SHARED_REFILL
+#define NF_SHARED_REFILL 1        // 1 (with NF_PRODUCER_WARP 0): any consumer warp refills the ring, under a lock; 0: warp 0 does
+#endif
+#ifndef NF_REFILL_BELOW
+#define NF_REFILL_BELOW 2          // a warp tries to refill when fewer than this many produced stages lie ahead of it
+#endif
 #define NF_CTA_THREADS ((NF_NW + NF_PRODUCER_WARP) * 32)
 #ifndef NF_SINKS
 #define NF_SINKS 2                // sinks per consumer thread (adjacent slots 2t, 2t+1 of the warp's range when 2)
@@ -36,7 +42,7 @@
 #endif
 #define NF_TABMAX 31              // source cells per segment table (32 entries = one per producer lane)
 #ifndef NF_NSTAGE
-#define NF_NSTAGE 4               // pipeline depth
+#define NF_NSTAGE 5               // pipeline depth
 #endif
 #ifndef NF_CELL_PAD
 #define NF_CELL_PAD 4             // every cell is padded to a multiple of this many slots (power of two, >= 2)

@@ -235,6 +235,7 @@ struct __align__(128) Stage {
 struct ProdState {       // cursor of the stage producer (block, column, z-run, chunk), kept in shared memory
     int mode;            // 0 next block, 1 next z-run, 5 z-run requested, 2 next chunk of the run, 3 end of block, 4 finished
     int flags, a, b, u, U1, Z1, ci, cj, ucur, run;
+    int owner;           // warp whose register holds the requested table (NF_SHARED_REFILL)
     uint32_t col, s0, cnt, c0, ge;
 };
 
@@ -563,6 +564,15 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
     // no registers in the pair loop.  produce_one() emits exactly one stage.
     __shared__ ProdState ps;
     __shared__ uint32_t ptab[32];
+#if NF_SHARED_REFILL
+    // Any warp may refill: the one that gets to a stage boundary with room in the ring takes a lock
+    // and emits stages, so the warps that would otherwise wait for data do the production work.
+    __shared__ volatile uint32_t nprod_sh;     // stages produced so far
+    __shared__ volatile int pdone_sh;          // the EXIT stage has been emitted
+    __shared__ int plock;
+    uint32_t cons = 0;                         // stages this warp has consumed
+    if (threadIdx.x == 0) { nprod_sh = 0u; pdone_sh = 0; plock = 0; ps.owner = -1; }
+#endif
     if (threadIdx.x == 0) { ps.mode = 0; ps.flags = 0; }
     __syncthreads();
     int pstage = 0, ahead = 0;
@@ -588,6 +598,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
         q.ucur = q.u; q.run = run;
         q.u += run;
         q.mode = 5;
+        q.owner = warp;
     };
     auto produce_one = [&]() -> bool {
         Stage &S = stages[pstage];
@@ -632,6 +643,13 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
             }
             if (q.mode == 1) issue_run(q);           // (only right after a block start or an empty run: not prefetched)
             if (q.mode == 5) {                       // the run's table has been requested: is the run non-empty?
+#if NF_SHARED_REFILL
+                if (q.owner != warp) {               // requested by another warp: fetch it again (cache-hot by now)
+                    int ia; const int sci = nf_wrap1(q.ci + q.a, cpd, ia);
+                    int ib; const int scj = nf_wrap1(q.cj + q.b, cpd, ib);
+                    tvp = A.poff[(sci * cpd + scj) * cpd + nf_mod(q.ucur, cpd) + (lane <= q.run ? lane : q.run)];
+                }
+#endif
                 const uint32_t g0 = __shfl_sync(0xffffffffu, tvp, 0);
                 const uint32_t g1 = __shfl_sync(0xffffffffu, tvp, q.run);
                 if (g1 <= g0) { q.mode = 1; continue; }
@@ -686,6 +704,39 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
 
     for (;;) {
 #if !NF_PRODUCER_WARP
+#if NF_SHARED_REFILL
+        while (!pdone_sh) {
+            uint32_t np = nprod_sh;
+            np = __shfl_sync(0xffffffffu, np, 0);
+            if (np - cons >= (uint32_t)NF_REFILL_BELOW) break;              // enough stages ahead of this warp (or the ring is full)
+            int got = 0;
+            if (lane == 0) got = (atomicCAS(&plock, 0, 1) == 0) ? 1 : 0;
+            got = __shfl_sync(0xffffffffu, got, 0);
+            if (!got) { if (np == cons) continue; else break; }              // someone else is refilling; spin only if starved
+            __threadfence_block();
+            np = nprod_sh;
+            np = __shfl_sync(0xffffffffu, np, 0);
+            bool released = false;
+            if (!pdone_sh && np - cons < (uint32_t)NF_NSTAGE) {
+                pstage = (int)(np % NF_NSTAGE);
+                pphase = (np / NF_NSTAGE) & 1u;
+                bool ok = mbar_test(&empty_bar[pstage], pphase ^ 1u);
+                if (!ok && np == cons) { mbar_wait<0>(&empty_bar[pstage], pphase ^ 1u); ok = true; }   // starved: wait for the slot
+                if (ok) {
+                    const bool last = produce_one();
+                    if (lane == 0) { if (last) pdone_sh = 1; __threadfence_block(); nprod_sh = np + 1u; }
+                    __syncwarp();
+                } else {
+                    released = true;          // slot still in use and there is something to consume: try again later
+                }
+            } else {
+                released = true;
+            }
+            if (lane == 0) { __threadfence_block(); atomicExch(&plock, 0); }
+            __syncwarp();
+            if (released) break;
+        }
+#else
         if (warp == 0 && !pdone) {
             // refill every free slot; block only when there is nothing left to consume
             while (ahead < NF_NSTAGE) {
@@ -697,6 +748,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                 if (pdone) break;
             }
         }
+#endif
 #endif
         Stage &S = stages[stage];
         mbar_wait<NF_CONSUMER_SLEEP_NS>(&full_bar[stage], phase);
@@ -844,7 +896,11 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
         if (lane == 0) mbar_arrive(&empty_bar[stage]);
         if (++stage == NF_NSTAGE) { stage = 0; phase ^= 1u; }
 #if !NF_PRODUCER_WARP
+#if NF_SHARED_REFILL
+        ++cons;
+#else
         --ahead;
+#endif
 #endif
     }
 }
