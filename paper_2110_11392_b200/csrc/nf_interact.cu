@@ -17,9 +17,10 @@
 //     slots or the LSU;
 //   * source cells that cannot hold r < eps_s skip the spline (11 instead of 14 FMA-pipe ops);
 //     with a close-pair radius the near cells clamp r^-3 and close_scan repairs close pairs in double;
-//   * no producer warp: consumer warp 0 refills the NF_NSTAGE-deep full/empty mbarrier ring of
-//     (column, z-run, chunk) stages from a cursor in shared memory; persistent CTAs pull sink
-//     blocks from an atomic counter in grid order;
+//   * no producer warp: the consumer warps refill the NF_NSTAGE-deep full/empty mbarrier ring of
+//     (column, z-run, chunk) stages themselves, from a cursor in shared memory and under a lock
+//     (whichever warp runs ahead does it); persistent CTAs pull sink blocks from an atomic
+//     counter in grid order;
 //   * A6 is fused: each thread writes gm/cell^2 * a straight to d_acc[perm[slot]].
 #include "nf_common.cuh"
 
@@ -559,9 +560,10 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
 #else
     // =========================== production by consumer warp 0 ================================
     // No dedicated producer warp: its registers go to the consumers (4 CTAs x 4 warps x 128
-    // registers fill the register file).  Warp 0 refills freed ring slots at its stage
-    // boundaries; the (block, column, z-run, chunk) cursor lives in shared memory so that it costs
-    // no registers in the pair loop.  produce_one() emits exactly one stage.
+    // registers fill the register file).  Consumer warps refill freed ring slots at their stage
+    // boundaries (NF_SHARED_REFILL: any warp with little produced work ahead of it, under a lock;
+    // else warp 0); the (block, column, z-run, chunk) cursor lives in shared memory so that it
+    // costs no registers in the pair loop.  produce_one() emits exactly one stage.
     __shared__ ProdState ps;
     __shared__ uint32_t ptab[32];
 #if NF_SHARED_REFILL
