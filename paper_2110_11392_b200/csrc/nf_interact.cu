@@ -862,8 +862,10 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                     // the common length of the two cells, both lane groups at once; then the rest of
                     // the longer cell, its own lanes only
                     if (ncm > 0) pass(a0, cA, b0, cB, ncm, mA > mB ? mA : mB);
-                    if (nA > ncm) pass(a0 + ncm, cA, 0, -(1 << 28), nA - ncm, mA);
-                    else if (nB > ncm) pass(b0 + ncm, cB, 0, -(1 << 28), nB - ncm, mB);
+                    if (nA != nB) {       // one call site for either remainder keeps the kernel's code (and its i-cache footprint) smaller
+                        const bool ra = nA > nB;
+                        pass((ra ? a0 : b0) + ncm, ra ? cA : cB, 0, -(1 << 28), ra ? nA - ncm : nB - ncm, ra ? mA : mB);
+                    }
                 }
             }
 #pragma unroll
