@@ -269,6 +269,8 @@ def main():
 
     # ------------------------------------------------------------------ our arm
     import torch
+    from paper_2110_11392_b200.build import ensure_built
+    ensure_built()                                   # no-op unless the .so is missing (fresh checkout)
     from paper_2110_11392_b200.binding import NearField, probe_pipes
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")

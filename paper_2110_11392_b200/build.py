@@ -39,5 +39,11 @@ def build_library(force: bool = False, verbose: bool = False, out: str | None = 
     return lib
 
 
+def ensure_built() -> str:
+    """Build the library only if the .so is missing (a fresh checkout: the .so is not tracked).
+    A build step, not a fallback: without nvcc this raises."""
+    return LIB if os.path.exists(LIB) else build_library(force=True)
+
+
 if __name__ == "__main__":
     print(build_library(force="--force" in sys.argv, verbose="-v" in sys.argv))

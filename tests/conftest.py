@@ -12,6 +12,13 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 
 
+@pytest.fixture(scope="session", autouse=True)
+def _library_built():
+    """a fresh checkout has no .so (it is not tracked): compile it once (nvcc) before any test loads it"""
+    from paper_2110_11392_b200.build import ensure_built
+    ensure_built()
+
+
 @pytest.fixture(scope="session")
 def oracle_mod():
     import oracle
