@@ -23,7 +23,7 @@
  * piecewise Eq. 3 with a branch (not the GPU's min form), no blocking, no reordering beyond
  * the loop nest "sink cell -> (a,b,c) lexicographic -> sink -> source".
  *
- * Parity pins (tests/test_oracle_pins.py): two-particle closed form inside/outside eps_s,
+ * Parity pins (tests/test_oracle_pins.py; variants incl. the unsoftened law: tests/test_oracle_variant_pins.py): two-particle closed form inside/outside eps_s,
  * cell-based cutoff, periodic wrap, one-particle-per-cell lattice => 0, momentum sum = 0,
  * all-pairs brute force masked to near-field cell pairs, integer pair-count identity,
  * CPD = 2R+1 => plain all-pairs, whole-cell translation, input-order invariance.
@@ -255,6 +255,9 @@ int64_t nfo_accel(const float *pos, int64_t N, int cpd, int R, double eps_p, dou
  * definition as nfo_accel:
  *   law = 0  spline softening, Eq. 3, eps_s = 2.16 eps_p
  *   law = 1  Plummer softening, Eq. 2: F = r / (r^2 + eps_p^2)^(3/2)
+ *   law = 2  no softening: "Newtonian gravity, or a softened form thereof", F = r/|r|^3;
+ *            eps_p is ignored; a coincident pair (r = 0) contributes 0, as F(0) = 0 does for
+ *            both softened laws (reading S4 carried over; reading N1)
  *   dens_b > 0 and dens != NULL: the FoF-scale density estimate of sec. 3.4.4,
  *       "an apodized top-hat density estimate 1 - r^2/b^2 (for r < b), which is computed as
  *       b^2 - r^2 on the GPU":   dens_p = sum over sources q != p of the same (2R+1)^3 cells
@@ -266,7 +269,7 @@ int64_t nfo_accel(const float *pos, int64_t N, int cpd, int R, double eps_p, dou
  */
 int64_t nfo_accel_variant(const float *pos, int64_t N, int cpd, int R, double eps_p, double box, double gm, int law, double dens_b,
                           const int32_t *sink_cells, int64_t n_sink_cells, double *acc, double *dens, int nthreads) {
-    if (N < 0 || R < 1 || cpd < 2 * R + 1 || !(eps_p > 0) || !(box > 0) || law < 0 || law > 1 || dens_b < 0) return -1;
+    if (N < 0 || R < 1 || cpd < 2 * R + 1 || !(eps_p > 0) || !(box > 0) || law < 0 || law > 2 || dens_b < 0) return -1;
     const int64_t ncell = (int64_t)cpd * cpd * cpd;
     const double cellsz = box / (double)cpd;
     const double eps_s = NFO_SPLINE_PER_PLUMMER * eps_p;
@@ -324,6 +327,8 @@ int64_t nfo_accel_variant(const float *pos, int64_t N, int cpd, int R, double ep
                                 if (law == 1) {
                                     const double s2 = r2 + eps_p * eps_p;    /* Eq. 2 */
                                     f = 1.0 / (s2 * sqrt(s2));
+                                } else if (law == 2) {
+                                    f = 1.0 / (r2 * sqrt(r2));               /* Newtonian */
                                 } else {
                                     const double r = sqrt(r2);
                                     if (r < eps_s) {

@@ -167,7 +167,8 @@ def accel(pos, cpd: int, R: int, eps_p: float, box: float = 1.0, gm: float | Non
 def accel_variant(pos, cpd: int, R: int, eps_p: float, box: float = 1.0, gm: float | None = None,
                   law: str = "spline", density_b: float = 0.0, sink_cells=None, nthreads: int = 0):
     """The build-time variants of the paper's kernel, by the definition:
-    ``law`` = "spline" (Eq. 3) or "plummer" (Eq. 2); ``density_b`` > 0 adds the
+    ``law`` = "spline" (Eq. 3), "plummer" (Eq. 2) or "newton" (no softening,
+    PAPER.md:218: r/|r|^3, coincident pairs contribute 0; eps_p ignored); ``density_b`` > 0 adds the
     FoF-scale density estimate sum_{q != p, r < b} (b^2 - r^2).
     -> (acc[N,3] float64, dens[N] float64 or None, pairs visited)."""
     p = _f32pos(pos)
@@ -182,7 +183,7 @@ def accel_variant(pos, cpd: int, R: int, eps_p: float, box: float = 1.0, gm: flo
         sc = np.ascontiguousarray(sink_cells, dtype=np.int32)
         sc_ptr, nsc = sc.ctypes.data, sc.shape[0]
     pairs = _load().nfo_accel_variant(p.ctypes.data, N, cpd, R, float(eps_p), float(box), float(gm),
-                                      {"spline": 0, "plummer": 1}[law], float(density_b), sc_ptr, nsc,
+                                      {"spline": 0, "plummer": 1, "newton": 2}[law], float(density_b), sc_ptr, nsc,
                                       acc.ctypes.data, dens.ctypes.data if dens is not None else None, int(nthreads))
     if pairs < 0:
         raise ValueError("nfo_accel_variant: bad arguments or non-finite position")

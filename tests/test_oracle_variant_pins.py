@@ -156,3 +156,72 @@ def test_W6_density_does_not_change_the_force():
     a0, _, p0 = oracle.accel_variant(pos, CPD, R, 0.01)
     a1, d1, p1 = oracle.accel_variant(pos, CPD, R, 0.01, density_b=0.04)
     assert np.array_equal(a0, a1) and p0 == p1 and d1 is not None
+
+
+# ---------------------------------------------------------------- no softening
+def test_N1_newton_two_particle_inverse_square():
+    """'Newtonian gravity, or a softened form thereof': |a| = gm / r^2 at every
+    separation, however small, attractive, a1 = -a2; along an oblique direction too."""
+    for sep in (1e-6, 1e-4, 0.003, 0.05, 0.2):
+        pos = _two(sep)
+        d = float(pos[1, 0]) - float(pos[0, 0])
+        acc, _, pairs = oracle.accel_variant(pos, CPD, R, 0.01, gm=2.5, law="newton")
+        assert pairs == 2
+        assert np.allclose(acc[0], [2.5 / d ** 2, 0, 0], rtol=1e-13, atol=0)
+        assert np.array_equal(acc[1], -acc[0])
+    p = np.array([[0.5, 0.5, 0.5], [0.5 + 0.02, 0.5 - 0.01, 0.5 + 0.02]], dtype=np.float32)
+    dv = p[1].astype(np.float64) - p[0].astype(np.float64)
+    acc, _, _ = oracle.accel_variant(p, CPD, R, 0.01, gm=1.0, law="newton")
+    assert np.allclose(acc[0], dv / np.linalg.norm(dv) ** 3, rtol=1e-12)
+
+
+def test_N2_newton_ignores_eps_and_is_the_limit_of_both_softened_laws():
+    """eps_p does not enter; Eq. 3 equals it exactly once every pair has r >= eps_s (compact
+    support); Eq. 2 approaches it as 1.5 (eps/r)^2."""
+    rng = np.random.default_rng(12)
+    pos = rng.random((300, 3)).astype(np.float32)
+    a_n, _, p_n = oracle.accel_variant(pos, CPD, R, 0.01, law="newton")
+    a_n2, _, _ = oracle.accel_variant(pos, CPD, R, 3.0, law="newton")
+    assert np.array_equal(a_n, a_n2)
+    x = pos.astype(np.float64)
+    dmin = min(np.sqrt((((x - x[i]) - np.round(x - x[i])) ** 2).sum(1))[np.arange(300) != i].min() for i in range(300))
+    eps = 0.4 * dmin / 2.16                                   # eps_s = 2.16 eps < every separation
+    a_s, _, p_s = oracle.accel_variant(pos, CPD, R, eps, law="spline")
+    assert p_s == p_n
+    assert np.abs(a_s - a_n).max() <= 1e-13 * np.abs(a_n).max()
+    a_p, _, _ = oracle.accel_variant(pos, CPD, R, 1e-7, law="plummer")
+    assert np.abs(a_p - a_n).max() <= 1e-6 * np.abs(a_n).max()
+    assert np.abs(a_n.sum(axis=0)).max() < 1e-13 * np.abs(a_n).sum()        # momentum
+
+
+def test_N3_newton_brute_force_all_pairs_masked():
+    rng = np.random.default_rng(6)
+    N = 500
+    pos = rng.random((N, 3)).astype(np.float32)
+    acc, _, pairs = oracle.accel_variant(pos, CPD, R, 0.02, gm=1.0 / N, law="newton")
+    x = pos.astype(np.float64)
+    cell = np.floor(x * CPD).astype(int) % CPD
+    ref = np.zeros((N, 3))
+    npairs = 0
+    for i in range(N):
+        d = x - x[i]
+        d -= np.round(d)
+        dc = (cell - cell[i] + CPD // 2) % CPD - CPD // 2
+        m = (np.abs(dc) <= R).all(axis=1)
+        m[i] = False
+        npairs += int(m.sum())
+        r2 = (d[m] ** 2).sum(axis=1)
+        ref[i] = (d[m] / r2[:, None] ** 1.5).sum(axis=0) / N
+    assert pairs == npairs
+    rms = np.sqrt((ref ** 2).sum(axis=1).mean())
+    assert np.abs(acc - ref).max() < 1e-12 * rms
+
+
+def test_N4_newton_coincident_particles_contribute_nothing():
+    """reading N1: F(0) = 0 for a coincident pair, as for the softened laws (S4) -- no Inf/NaN."""
+    pos = np.array([[0.3, 0.3, 0.3], [0.3, 0.3, 0.3], [0.35, 0.3, 0.3]], dtype=np.float32)
+    acc, _, pairs = oracle.accel_variant(pos, CPD, R, 0.01, gm=1.0, law="newton")
+    d = float(pos[2, 0]) - float(pos[0, 0])
+    assert pairs == 6 and np.isfinite(acc).all()
+    assert np.allclose(acc[0], [1 / d ** 2, 0, 0], rtol=1e-13) and np.array_equal(acc[0], acc[1])
+    assert np.allclose(acc[2], [-2 / d ** 2, 0, 0], rtol=1e-13)
