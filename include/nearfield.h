@@ -52,6 +52,7 @@ typedef enum {
 #define NF_MAX_MULTIPOLE_ORDER 16   /* compiled maximum order p of nf_multipoles */
 #define NF_SOFT_SPLINE 0    /* Eq. 3, the paper's "single_spline" (Fig. 19) */
 #define NF_SOFT_PLUMMER 1   /* Eq. 2 */
+#define NF_SOFT_NEWTON 2    /* no softening: F = r/|r|^3 ("Newtonian gravity, or a softened form thereof") */
 #define NF_N_STAGES 8       /* entries of nf_stage_ms */
 
 /*
@@ -90,10 +91,28 @@ nf_status nf_set_gm(nf_ctx *ctx, double gm);
 nf_status nf_accel(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc, void *cuda_stream);
 
 /*
+ * nf_bin -- run the binning (A1..A3) of d_pos now and KEEP it: until the particles move, every
+ * call on ctx that is given the same d_pos pointer and N (nf_accel, nf_accel4, nf_accel_f64,
+ * nf_multipoles, nf_taylor_accel, nf_timestep_ratio) reuses this grid order instead of sorting
+ * again -- within one time step the force, multipole, Taylor and time-step calls see the same
+ * positions (Table 1).  The caller promises not to change d_pos meanwhile.  The
+ * pin ends at the next nf_bin / nf_rebin / nf_unbin, at an nf_kick_drift of that buffer with
+ * dt_drift != 0, or when a call passes another buffer or count (which is then sorted as usual).
+ * NF_EINVAL: ctx/d_pos NULL, N <= 0 or too large.
+ */
+nf_status nf_bin(nf_ctx *ctx, const float *d_pos, int64_t N, void *cuda_stream);
+
+/* nf_unbin -- drop the pin of nf_bin (the next call sorts again). */
+nf_status nf_unbin(nf_ctx *ctx);
+
+/*
  * nf_set_softening -- the "near-force softening technique" the paper chooses at build time
  * (PAPER.md:620): NF_SOFT_SPLINE (default; Eq. 3 with eps_s = 2.16 eps_plummer) or
- * NF_SOFT_PLUMMER (Eq. 2, F = r/(r^2 + eps_plummer^2)^(3/2)).  Takes effect at the
- * next nf_accel / nf_accel4.  NF_EINVAL: ctx NULL or an unknown law.
+ * NF_SOFT_PLUMMER (Eq. 2, F = r/(r^2 + eps_plummer^2)^(3/2)) or NF_SOFT_NEWTON (no
+ * softening, F = r/|r|^3; eps_plummer is ignored, a coincident pair contributes 0 as
+ * F(0) = 0 does for the softened laws; pairs closer than the close-pair radius are evaluated in
+ * double precision, see option "rc_cells").  Takes effect at the next nf_accel / nf_accel4 /
+ * nf_accel_f64.  NF_EINVAL: ctx NULL or an unknown law.
  */
 nf_status nf_set_softening(nf_ctx *ctx, int law);
 
@@ -116,6 +135,28 @@ nf_status nf_set_density_radius(nf_ctx *ctx, double b);
  * [0, cpd), nx outside [1, cpd].
  */
 nf_status nf_set_sink_slabs(nf_ctx *ctx, int x0, int nx);
+
+/*
+ * Device-side support of the slab decomposition (paper_2110_11392_b200/slabs.py is the host plumbing
+ * around these; ghost slabs = near-field radius, Table 1):
+ *
+ * nf_cell_histogram -- occupancy histogram of N particles under step A1's cell rule (half-open cells,
+ *   periodic wrap of any finite position): d_counts [out] device, cpd^3 int32, key = (cx*cpd+cy)*cpd+cz,
+ *   caller-owned (so that ranks can sum their histograms with one all-reduce).  Zero-fills first;
+ *   N == 0 gives zeros.  A NaN/Inf position is not counted and makes the next nf_sync return NF_EPOS.
+ * nf_slab_pairs -- from a (global) histogram, per x slab i: d_npart[i] = particles in the slab and
+ *   d_pairs[i] = sum over its cells c of n_c * sum_{c' in N(c)} n_c' (self pairs included: subtract
+ *   d_npart for the q != p count), the integer identity P7 -- the work the slabs are balanced by.
+ *   d_pairs, d_npart [out] device, cpd int64 each.
+ * nf_select_slabs -- copy the particles whose x cell index lies in the periodic range [x0, x0 + nx)
+ *   to d_out (device, room for N*3 floats; NULL = count only) in input order, and return their number
+ *   in *h_count (synchronises the stream).  nx = 0 selects nothing.
+ * NF_EINVAL: NULL arguments, N < 0 or too large, x0 outside [0, cpd), nx outside [0, cpd].
+ */
+nf_status nf_cell_histogram(nf_ctx *ctx, const float *d_pos, int64_t N, int32_t *d_counts, void *cuda_stream);
+nf_status nf_slab_pairs(nf_ctx *ctx, const int32_t *d_counts, int64_t *d_pairs, int64_t *d_npart, void *cuda_stream);
+nf_status nf_select_slabs(nf_ctx *ctx, const float *d_pos, int64_t N, int x0, int nx, float *d_out, int64_t *h_count,
+                          void *cuda_stream);
 
 /*
  * nf_accel4 -- nf_accel with the accelerations "promoted to 4-vectors":
@@ -227,7 +268,11 @@ const char *nf_last_error(const nf_ctx *ctx);
  *   "rc_cells"     (<= 0.25) close-pair radius in cell units: pairs with r < rc are evaluated
  *                        exactly in double precision instead of the float32 fast path;
  *                        0 = none (Eq. 3 as a min everywhere); negative (default) = automatic,
- *                        from the particle-weighted occupancy and eps_s
+ *                        from the particle-weighted occupancy and eps_s.
+ *                        Spline law: a positive radius below eps_s is raised to eps_s (the fast
+ *                        path evaluates Eq. 3's polynomial only inside the close-pair radius, so the
+ *                        radius may not end inside the softened core); the value in
+ *                        force is what nf_close_radius reports.  NF_SOFT_NEWTON: at least 1e-4.
  * NF_EINVAL: unknown name or value out of range.
  */
 nf_status nf_set_option(nf_ctx *ctx, const char *name, double value);
@@ -269,29 +314,34 @@ nf_status nf_launch_count(nf_ctx *ctx, int64_t *h_count);
 nf_status nf_debug_read(nf_ctx *ctx, const void *d_src, void *h_dst, uint64_t bytes);
 
 /*
- * nf_debug_neighbors -- the neighbour list the interaction kernel's segment enumerator
- * visits for sink cell `cell`: (2R+1)^3 entries in (a,b,c) lexicographic order,
- * h_ids[n] = neighbour cell key, h_image[3n..3n+2] = periodic image counts in {-1,0,1}
- * (PAPER.md:218, :232).  Produced on the device by the same code the kernel runs.
+ * nf_debug_neighbors -- the neighbour list of sink cell `cell` under the enumeration rule of the
+ * interaction kernel's stage producer (column images by a single wrap, z by the modulus of the
+ * unwrapped index): (2R+1)^3 entries in (a,b,c) lexicographic order, h_ids[n] = neighbour cell
+ * key, h_image[3n..3n+2] = periodic image counts in {-1,0,1}.  Produced on
+ * the device by a separate one-thread kernel that restates that rule -- it checks the rule, not
+ * what the interaction kernel visited; nf_debug_delivered_pairs measures the latter.
  */
 nf_status nf_debug_neighbors(nf_ctx *ctx, int cell, int32_t *h_ids, int8_t *h_image);
 
 /*
- * nf_interaction_count -- pairs (sink, source), source != sink, of the last nf_accel:
- * sum_c n_c * sum_{c' in N(c)} n_c'  -  N, counted on the device from the cell offsets.
- * Padding and masked lanes are not work.  Synchronises.
+ * nf_debug_delivered_pairs -- what the interaction kernel's traversal DELIVERS, measured: re-runs
+ * the sink blocks of the last nf_accel / nf_accel4 through a counting instantiation of the
+ * interaction kernel (same copy ring, stage cursor, z-windows and paired-cell passes; the pair
+ * arithmetic replaced by a count of the non-padding sources each pass hands to each non-padding
+ * sink).  h_out[0] = (sink, source) deliveries including each sink's meeting with itself,
+ * h_out[1] = meetings of a sink with itself.  A correct traversal gives h_out[1] = number of
+ * sinks and h_out[0] - h_out[1] = nf_interaction_count = the oracle's pair count (pin P7).
+ * Synchronises.  NF_EINVAL: NULL arguments, or the last call on ctx was not nf_accel / nf_accel4.
  */
-nf_status nf_interaction_count(nf_ctx *ctx, int64_t *h_pairs);
+nf_status nf_debug_delivered_pairs(nf_ctx *ctx, int64_t *h_out /* 2 */);
 
 /*
- * nf_probe_pipes -- microbenchmarks that give the roofline denominators on this device:
- *   h_out[0] FP32 FMA-pipe lane-operations per second, scalar FFMA stream
- *   h_out[1] the same for packed fma.rn.f32x2 (two lanes per thread-instruction)
- *   h_out[2] MUFU.RSQ lane-operations per second
- *   h_out[3] SM count   h_out[4] SM clock (MHz) reported by the runtime
- * Runs on the current device, synchronises.  NF_EINVAL: h_out NULL.
+ * nf_interaction_count -- pairs (sink, source), source != sink, of the last nf_accel:
+ * sum_c n_c * sum_{c' in N(c)} n_c'  -  N, computed on the device from the cell offsets (the
+ * formula; nf_debug_delivered_pairs is the measurement).  Padding and masked lanes are not work.
+ * Synchronises.
  */
-nf_status nf_probe_pipes(double *h_out /* 5 */);
+nf_status nf_interaction_count(nf_ctx *ctx, int64_t *h_pairs);
 
 #ifdef __cplusplus
 }

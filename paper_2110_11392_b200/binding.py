@@ -21,8 +21,9 @@ STAGE_NAMES = ["A1_key_hist", "A2_scan", "A3_scatter_rank_gather", "A4_scheduler
 # every symbol include/nearfield.h declares
 SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", "nf_sync",
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
-           "nf_interaction_count", "nf_probe_pipes", "nf_debug_read", "nf_launch_count", "nf_close_radius",
-           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles", "nf_kick_drift", "nf_timestep_ratio", "nf_taylor_accel"]
+           "nf_interaction_count", "nf_debug_read", "nf_launch_count", "nf_close_radius",
+           "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles", "nf_kick_drift", "nf_timestep_ratio", "nf_taylor_accel",
+           "nf_debug_delivered_pairs", "nf_bin", "nf_unbin", "nf_cell_histogram", "nf_slab_pairs", "nf_select_slabs"]
 
 
 class NearFieldError(RuntimeError):
@@ -32,8 +33,8 @@ class NearFieldError(RuntimeError):
 
 
 def lib_path() -> str:
-    """the in-tree library, or the build named by NEARFIELD_B200_LIB (a tuning variant)"""
-    return os.environ.get("NEARFIELD_B200_LIB") or os.path.join(_HERE, "libnearfield_b200.so")
+    """the in-tree library"""
+    return os.path.join(_HERE, "libnearfield_b200.so")
 
 
 def load_library() -> ctypes.CDLL:
@@ -86,28 +87,28 @@ def load_library() -> ctypes.CDLL:
     L.nf_debug_neighbors.argtypes = [vp, i32, vp, vp]
     L.nf_interaction_count.restype = i32
     L.nf_interaction_count.argtypes = [vp, ctypes.POINTER(i64)]
+    L.nf_debug_delivered_pairs.restype = i32
+    L.nf_debug_delivered_pairs.argtypes = [vp, vp]
+    L.nf_bin.restype = i32
+    L.nf_bin.argtypes = [vp, vp, i64, vp]
+    L.nf_unbin.restype = i32
+    L.nf_unbin.argtypes = [vp]
+    L.nf_cell_histogram.restype = i32
+    L.nf_cell_histogram.argtypes = [vp, vp, i64, vp, vp]
+    L.nf_slab_pairs.restype = i32
+    L.nf_slab_pairs.argtypes = [vp, vp, vp, vp, vp]
+    L.nf_select_slabs.restype = i32
+    L.nf_select_slabs.argtypes = [vp, vp, i64, i32, i32, vp, ctypes.POINTER(i64), vp]
     L.nf_close_radius.restype = i32
     L.nf_close_radius.argtypes = [vp, ctypes.POINTER(dbl)]
     L.nf_launch_count.restype = i32
     L.nf_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     L.nf_debug_read.restype = i32
     L.nf_debug_read.argtypes = [vp, vp, vp, ctypes.c_uint64]
-    L.nf_probe_pipes.restype = i32
-    L.nf_probe_pipes.argtypes = [vp]
     return L
 
 
 _L = load_library()
-
-
-def probe_pipes() -> dict:
-    """nf_probe_pipes: measured FP32-FMA / packed-FMA / MUFU.RSQ lane rates of the device."""
-    out = (ctypes.c_double * 5)()
-    rc = _L.nf_probe_pipes(out)
-    if rc != NF_OK:
-        raise NearFieldError(rc, "nf_probe_pipes")
-    return {"ffma_lane_ops_per_s": out[0], "ffma2_lane_ops_per_s": out[1], "mufu_rsq_lane_ops_per_s": out[2],
-            "sm_count": int(out[3]), "sm_clock_mhz": out[4]}
 
 
 class NearField:
@@ -168,12 +169,63 @@ class NearField:
         return acc
 
     def set_softening(self, law: str):
-        """"spline" (Eq. 3, default) or "plummer" (Eq. 2) -- nf_set_softening"""
-        self._check(_L.nf_set_softening(self._h, {"spline": 0, "plummer": 1}[law]))
+        """"spline" (Eq. 3, default), "plummer" (Eq. 2) or "newton" (no softening) -- nf_set_softening"""
+        self._check(_L.nf_set_softening(self._h, {"spline": 0, "plummer": 1, "newton": 2}[law]))
+
+    def bin(self, pos, stream=None):
+        """nf_bin: sort ``pos`` into grid order now and keep the binning for the following calls on ``pos``."""
+        import torch
+        if not (pos.is_cuda and pos.dtype == torch.float32 and pos.is_contiguous() and pos.dim() == 2 and pos.shape[1] == 3):
+            raise ValueError("pos must be a contiguous CUDA float32 tensor of shape [N,3]")
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        self._N = pos.shape[0]
+        self._check(_L.nf_bin(self._h, pos.data_ptr(), pos.shape[0], ctypes.c_void_p(st.cuda_stream)))
+
+    def unbin(self):
+        self._check(_L.nf_unbin(self._h))
+
+    def delivered_pairs(self):
+        """nf_debug_delivered_pairs -> (deliveries incl. self meetings, self meetings) of the last accel."""
+        out = (ctypes.c_int64 * 2)()
+        self._check(_L.nf_debug_delivered_pairs(self._h, out))
+        return int(out[0]), int(out[1])
 
     def set_sink_slabs(self, x0: int, nx: int):
         """only particles in x slabs [x0, x0 + nx) (periodic) are sinks -- nf_set_sink_slabs"""
         self._check(_L.nf_set_sink_slabs(self._h, int(x0), int(nx)))
+
+    def cell_histogram(self, pos, stream=None):
+        """nf_cell_histogram -> int32 [cpd^3] on the device (summable across ranks with all_reduce)."""
+        import torch
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        counts = torch.empty(self.cpd ** 3, dtype=torch.int32, device=pos.device)
+        N = pos.shape[0]
+        self._check(_L.nf_cell_histogram(self._h, pos.data_ptr() if N else None, N, counts.data_ptr(), ctypes.c_void_p(st.cuda_stream)))
+        return counts
+
+    def slab_pairs(self, counts, stream=None):
+        """nf_slab_pairs -> (pairs int64 [cpd], particles int64 [cpd]) per x slab, on the device."""
+        import torch
+        if not (counts.is_cuda and counts.dtype == torch.int32 and counts.is_contiguous() and counts.numel() == self.cpd ** 3):
+            raise ValueError("counts must be a contiguous CUDA int32 tensor of cpd^3 entries")
+        st = torch.cuda.current_stream(counts.device) if stream is None else stream
+        pairs = torch.empty(self.cpd, dtype=torch.int64, device=counts.device)
+        npart = torch.empty(self.cpd, dtype=torch.int64, device=counts.device)
+        self._check(_L.nf_slab_pairs(self._h, counts.data_ptr(), pairs.data_ptr(), npart.data_ptr(), ctypes.c_void_p(st.cuda_stream)))
+        return pairs, npart
+
+    def select_slabs(self, pos, x0: int, nx: int, out=None, stream=None) -> int:
+        """nf_select_slabs: particles of ``pos`` in x slabs [x0, x0+nx) (periodic) -> first rows of ``out``
+        ([>=count, 3] CUDA float32, input order kept); returns the count.  ``out`` None: count only."""
+        import torch
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        N = pos.shape[0]
+        if out is not None and not (out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.numel() >= 3 * N):
+            raise ValueError("out must be a contiguous CUDA float32 tensor with room for all of pos")
+        n = ctypes.c_int64()
+        self._check(_L.nf_select_slabs(self._h, pos.data_ptr() if N else None, N, int(x0), int(nx),
+                                       out.data_ptr() if out is not None else None, ctypes.byref(n), ctypes.c_void_p(st.cuda_stream)))
+        return int(n.value)
 
     def set_density_radius(self, b: float):
         self._check(_L.nf_set_density_radius(self._h, float(b)))

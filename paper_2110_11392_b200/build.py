@@ -1,48 +1,105 @@
-"""Build step: compile ``csrc/*.cu`` into ``libnearfield_b200.so`` in-tree with nvcc for sm_100a.
+"""Build step: compile ``csrc/*.cu`` with nvcc for sm_100a, in-tree.
 
-``python -m paper_2110_11392_b200.build`` (or ``__graft_entry__.build()``).  nvcc
-cross-compiles without a GPU.  The .so is git-ignored but travels with the repo snapshot.
+``python -m paper_2110_11392_b200.build`` (or ``__graft_entry__.build()``) makes
+
+* ``libnearfield_b200.so`` -- the product: the C ABI of ``include/nearfield.h``;
+* ``libnf_pipeprobe.so``   -- a bench-only helper (``csrc/probe/nf_pipeprobe.cu``): FP32 / FP64 / MUFU
+  pipe-rate microbenchmarks that give ``bench.py`` its live roofline denominators.  Not part of the
+  product ABI.
+
+nvcc cross-compiles without a GPU.  The .so files are git-ignored but travel with the repo snapshot.
+Translation units are compiled in parallel and linked once.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnearfield_b200.so")
-SOURCES = ["nf_api.cu", "nf_binner.cu", "nf_interact.cu", "nf_f64.cu", "nf_multipoles.cu", "nf_taylor.cu", "nf_step.cu", "nf_probe.cu"]
+PROBE_LIB = os.path.join(HERE, "libnf_pipeprobe.so")
+SOURCES = ["nf_api.cu", "nf_binner.cu", "nf_interact.cu", "nf_f64.cu", "nf_multipoles.cu", "nf_taylor.cu", "nf_step.cu",
+           "nf_slabs.cu"]
+PROBE_SOURCES = [os.path.join("probe", "nf_pipeprobe.cu")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "-Xcompiler", "-Wno-format-truncation"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-Wno-format-truncation"]
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+def _deps() -> list[str]:
+    d = []
+    for root, _, files in os.walk(CSRC):
+        d += [os.path.join(root, f) for f in files]
+    return d + [os.path.join(HERE, "..", "include", "nearfield.h")]
+
+
+def _source_hash() -> str:
+    """content hash of every source and header (mtimes do not survive a copy of the tree)"""
+    import hashlib
+    h = hashlib.sha1()
+    for d in sorted(_deps()):
+        h.update(os.path.relpath(d, HERE).encode())
+        with open(d, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
+def _stale(lib: str) -> bool:
+    """missing, or built from other sources than the ones in the tree now"""
+    try:
+        with open(lib + ".srchash") as f:
+            return not os.path.exists(lib) or f.read().strip() != _source_hash()
+    except OSError:
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "nearfield.h")]
-    return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False, out: str | None = None, defines: tuple = ()) -> str:
-    """Compile the library.  ``out`` / ``defines`` build a tuning variant (-DNAME=VALUE for the
-    knobs of csrc/nf_common.cuh) somewhere else; the default build is the product."""
-    lib = out or LIB
-    if force or out is not None or _stale():
-        nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, *[f"-D{d}" for d in defines], "-o", lib + ".tmp", *[os.path.join(CSRC, s) for s in SOURCES]]
-        if verbose:
-            cmd.insert(1, "-Xptxas=-v")
-        subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
-        os.replace(lib + ".tmp", lib)
-    return lib
+def _compile(sources: list[str], lib: str, verbose: bool) -> None:
+    nvcc = os.environ.get("NVCC", "nvcc")
+    os.makedirs(OBJ, exist_ok=True)
+    headers = [d for d in _deps() if d.endswith((".cuh", ".h"))]
+    newest_header = max(os.path.getmtime(h) for h in headers)
+
+    def one(src: str) -> str:
+        path = os.path.join(CSRC, src)
+        obj = os.path.join(OBJ, src.replace(os.sep, "_") + ".o")
+        if not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(path), newest_header):
+            cmd = [nvcc, *NVCC_FLAGS, "-c", "-o", obj, path]
+            if verbose:
+                cmd.insert(1, "-Xptxas=-v")
+            subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(8, len(sources))) as ex:
+        objs = list(ex.map(one, sources))
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", lib + ".tmp", *objs],
+                   check=True, stdout=sys.stderr, stderr=sys.stderr)
+    os.replace(lib + ".tmp", lib)
+    with open(lib + ".srchash", "w") as f:
+        f.write(_source_hash() + "\n")
+
+
+def build_library(force: bool = False, verbose: bool = False) -> str:
+    """Compile both libraries if a source or header is newer than them (or ``force``)."""
+    if force:
+        for f in os.listdir(OBJ) if os.path.isdir(OBJ) else []:
+            os.remove(os.path.join(OBJ, f))
+    if force or _stale(LIB):
+        _compile(SOURCES, LIB, verbose)
+    if force or _stale(PROBE_LIB):
+        _compile(PROBE_SOURCES, PROBE_LIB, verbose)
+    return LIB
 
 
 def ensure_built() -> str:
-    """Build the library only if the .so is missing (a fresh checkout: the .so is not tracked).
-    A build step, not a fallback: without nvcc this raises."""
-    return LIB if os.path.exists(LIB) else build_library(force=True)
+    """Make sure the in-tree libraries exist and are not older than their sources (a fresh checkout
+    has none: they are not tracked).  A build step, not a fallback: without nvcc a stale or missing
+    library raises instead of being loaded silently."""
+    if _stale(LIB) or _stale(PROBE_LIB):
+        build_library()
+    return LIB
 
 
 if __name__ == "__main__":

@@ -64,6 +64,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
         return fail(NF_ENOMEM);                                                                 \
     }
     const size_t nscan = (size_t)((c->ncell + 2047) / 2048 + 8);
+    c->capScan = (int64_t)nscan;
     TRY_ALLOC(c->d_counts, (size_t)(c->ncell + 1) * 4);
     TRY_ALLOC(c->d_offsets, (size_t)(c->ncell + 1) * 4);
     TRY_ALLOC(c->d_poff, (size_t)(c->ncell + 1) * 4);
@@ -109,6 +110,7 @@ extern "C" nf_status nf_set_option(nf_ctx *c, const char *name, double v) {
     if (!c || !name) return NF_EINVAL;
     const int iv = (int)v;
     if (!strcmp(name, "rc_cells")) {
+        // (for the spline law a positive value below eps_s is raised to eps_s on the device: k_choose_rc)
         if (!(v <= 0.25) || !isfinite(v)) { snprintf(c->err, sizeof c->err, "nf_set_option(rc_cells): need value <= 0.25 (negative = automatic)"); return NF_EINVAL; }
         c->opt_rc = (float)v;
         return NF_OK;
@@ -125,6 +127,19 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
     if (N <= c->capN) return NF_OK;
     cudaStreamSynchronize(c->last_stream);
     free_scratch(c);
+    c->bin_pinned = 0; c->have_sched = 0;
+    {   // block totals of the scans: over the cells, and over N/256 selection blocks (nf_select_slabs)
+        const int64_t need = ((N + 255) / 256 + 2047) / 2048 + 8;
+        if (need > c->capScan) {
+            cudaFree(c->d_scan_blk); c->d_scan_blk = nullptr; c->capScan = 0;
+            if (cudaMalloc((void **)&c->d_scan_blk, (size_t)need * 8) != cudaSuccess) {
+                cudaGetLastError();
+                snprintf(c->err, sizeof c->err, "scratch allocation for N=%lld failed", (long long)N);
+                return NF_ENOMEM;
+            }
+            c->capScan = need;
+        }
+    }
     const int64_t capPad = ((N + (NF_CELL_PAD - 1) * c->ncell + 8 + 3) / 4) * 4 + 8;
     const int64_t capBlk = capPad / NF_BS + c->ncol + 8;
     cudaError_t e = cudaSuccess;
@@ -147,9 +162,42 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
     return NF_OK;
 }
 
+// A1..A3 for (d_pos, N), or nothing when nf_bin pinned a binning of exactly this buffer
+// ("most particles stay in their cell" -- and between the force, multipole, Taylor and
+// time-step calls of one step none moves at all).
+static nf_status bin_for(nf_ctx *c, const float *d_pos, int64_t N, cudaStream_t st) {
+    nf_status rc = ensure_scratch(c, N);
+    if (rc != NF_OK) return rc;
+    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    if (c->bin_pinned && c->bin_pos == d_pos && c->bin_N == N) return NF_OK;
+    c->bin_pinned = 0; c->have_sched = 0;
+    return nf_run_binner(c, d_pos, N, st);
+}
+
+extern "C" nf_status nf_bin(nf_ctx *c, const float *d_pos, int64_t N, void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N <= 0 || !d_pos || (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_bin: bad argument (N=%lld)", (long long)N);
+        return NF_EINVAL;
+    }
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    c->bin_pinned = 0;
+    nf_status rc = bin_for(c, d_pos, N, (cudaStream_t)cuda_stream);
+    if (rc != NF_OK) return rc;
+    c->bin_pinned = 1; c->bin_pos = d_pos; c->bin_N = N;
+    return NF_OK;
+}
+
+extern "C" nf_status nf_unbin(nf_ctx *c) {
+    if (!c) return NF_EINVAL;
+    c->bin_pinned = 0;
+    return NF_OK;
+}
+
 extern "C" nf_status nf_set_softening(nf_ctx *c, int law) {
     if (!c) return NF_EINVAL;
-    if (law != NF_SOFT_SPLINE && law != NF_SOFT_PLUMMER) { snprintf(c->err, sizeof c->err, "nf_set_softening: unknown law %d", law); return NF_EINVAL; }
+    if (law != NF_SOFT_SPLINE && law != NF_SOFT_PLUMMER && law != NF_SOFT_NEWTON) { snprintf(c->err, sizeof c->err, "nf_set_softening: unknown law %d", law); return NF_EINVAL; }
     c->law = law;
     return NF_OK;
 }
@@ -161,6 +209,47 @@ extern "C" nf_status nf_set_sink_slabs(nf_ctx *c, int x0, int nx) {
         return NF_EINVAL;
     }
     c->slab_x0 = x0; c->slab_nx = nx;
+    return NF_OK;
+}
+
+extern "C" nf_status nf_cell_histogram(nf_ctx *c, const float *d_pos, int64_t N, int32_t *d_counts, void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N < 0 || !d_counts || (N > 0 && !d_pos) || N >= 2147483647ll) { snprintf(c->err, sizeof c->err, "nf_cell_histogram: bad argument (N=%lld)", (long long)N); return NF_EINVAL; }
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    c->last_stream = (cudaStream_t)cuda_stream; c->have_last = 1;
+    return nf_run_cell_histogram(c, d_pos, N, d_counts, (cudaStream_t)cuda_stream);
+}
+
+extern "C" nf_status nf_slab_pairs(nf_ctx *c, const int32_t *d_counts, int64_t *d_pairs, int64_t *d_npart, void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (!d_counts || !d_pairs || !d_npart) { snprintf(c->err, sizeof c->err, "nf_slab_pairs: NULL argument"); return NF_EINVAL; }
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    return nf_run_slab_pairs(c, d_counts, (long long *)d_pairs, (long long *)d_npart, (cudaStream_t)cuda_stream);
+}
+
+extern "C" nf_status nf_select_slabs(nf_ctx *c, const float *d_pos, int64_t N, int x0, int nx, float *d_out, int64_t *h_count, void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N < 0 || !h_count || (N > 0 && !d_pos) || x0 < 0 || x0 >= c->cpd || nx < 0 || nx > c->cpd ||
+        (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_select_slabs: bad argument (N=%lld x0=%d nx=%d)", (long long)N, x0, nx);
+        return NF_EINVAL;
+    }
+    *h_count = 0;
+    if (N == 0 || nx == 0) return NF_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    nf_status rc = ensure_scratch(c, N);
+    if (rc != NF_OK) return rc;
+    c->last_stream = st; c->have_last = 1; c->have_sched = 0;      // (the block scan reuses ctrl[1])
+    rc = nf_run_select_slabs(c, d_pos, N, x0, nx, d_out, c->d_key, st);
+    if (rc != NF_OK) return rc;
+    uint32_t tot = 0;
+    NF_CUDA_OK(c, cudaMemcpyAsync(&tot, c->d_ctrl + 1, sizeof tot, cudaMemcpyDeviceToHost, st));
+    NF_CUDA_OK(c, cudaStreamSynchronize(st));
+    *h_count = (int64_t)tot;
     return NF_OK;
 }
 
@@ -181,12 +270,10 @@ static nf_status accel_any(nf_ctx *c, const float *d_pos, int64_t N, float *d_ac
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (N == 0) return NF_OK;
     NF_CUDA_OK(c, cudaSetDevice(c->device));
-    nf_status rc = ensure_scratch(c, N);
+    if (c->opt_stage_timing) { for (int i = 0; i < 4; ++i) cudaEventRecord(c->ev[i], st); cudaEventRecord(c->ev[6], st); }
+    nf_status rc = bin_for(c, d_pos, N, st);
     if (rc != NF_OK) return rc;
-    c->last_stream = st; c->lastN = N; c->have_last = 1;
-    if (c->opt_stage_timing) cudaEventRecord(c->ev[6], st);
-    rc = nf_run_binner(c, d_pos, N, st);
-    if (rc != NF_OK) return rc;
+    if (c->opt_stage_timing && c->bin_pinned) cudaEventRecord(c->ev[3], st);      // binning reused: stages A1-A3 read 0
     rc = nf_run_scheduler(c, N, st);
     if (rc != NF_OK) return rc;
     if (c->opt_stage_timing) cudaEventRecord(c->ev[4], st);
@@ -195,6 +282,7 @@ static nf_status accel_any(nf_ctx *c, const float *d_pos, int64_t N, float *d_ac
     const float kfac = (float)(gm / (cellsz * cellsz));
     rc = nf_run_interact(c, d_pos, N, d_acc, ostride, kfac, st);
     if (rc != NF_OK) return rc;
+    c->have_sched = 1;
     if (c->opt_stage_timing) { cudaEventRecord(c->ev[5], st); cudaEventRecord(c->ev[7], st); }
     return NF_OK;
 }
@@ -217,10 +305,7 @@ extern "C" nf_status nf_accel_f64(nf_ctx *c, const float *d_pos, int64_t N, doub
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (N == 0) return NF_OK;
     NF_CUDA_OK(c, cudaSetDevice(c->device));
-    nf_status rc = ensure_scratch(c, N);
-    if (rc != NF_OK) return rc;
-    c->last_stream = st; c->lastN = N; c->have_last = 1;
-    rc = nf_run_binner(c, d_pos, N, st);
+    nf_status rc = bin_for(c, d_pos, N, st);
     if (rc != NF_OK) return rc;
     return nf_run_f64(c, d_pos, N, d_acc, st);
 }
@@ -240,10 +325,7 @@ extern "C" nf_status nf_multipoles(nf_ctx *c, const float *d_pos, int64_t N, int
         NF_CUDA_OK(c, cudaMemsetAsync(d_M, 0, (size_t)c->ncell * cml * sizeof(double), st));
         return NF_OK;
     }
-    nf_status rc = ensure_scratch(c, N);
-    if (rc != NF_OK) return rc;
-    c->last_stream = st; c->lastN = N; c->have_last = 1;
-    rc = nf_run_binner(c, d_pos, N, st);
+    nf_status rc = bin_for(c, d_pos, N, st);
     if (rc != NF_OK) return rc;
     return nf_run_multipoles(c, d_pos, order, d_M, st);
 }
@@ -258,6 +340,7 @@ extern "C" nf_status nf_kick_drift(nf_ctx *c, float *d_pos, float *d_vel, const 
     }
     if (N == 0) return NF_OK;
     NF_CUDA_OK(c, cudaSetDevice(c->device));
+    if (c->bin_pinned && c->bin_pos == d_pos && dt_drift != 0.0) c->bin_pinned = 0;    // the particles move: re-sort (or nf_bin) next time
     return nf_run_kick_drift(c, d_pos, d_vel, d_acc, N, dt_kick, dt_drift, (cudaStream_t)cuda_stream);
 }
 
@@ -274,10 +357,7 @@ extern "C" nf_status nf_timestep_ratio(nf_ctx *c, const float *d_pos, const floa
     if (N == 0) return NF_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     NF_CUDA_OK(c, cudaSetDevice(c->device));
-    nf_status rc = ensure_scratch(c, N);
-    if (rc != NF_OK) return rc;
-    c->last_stream = st; c->lastN = N; c->have_last = 1;
-    rc = nf_run_binner(c, d_pos, N, st);
+    nf_status rc = bin_for(c, d_pos, N, st);
     if (rc != NF_OK) return rc;
     double *d3 = (double *)(c->d_pairs + 2);
     rc = nf_run_timestep_ratio(c, d_vel, d_acc, d3, st);
@@ -304,10 +384,7 @@ extern "C" nf_status nf_taylor_accel(nf_ctx *c, const float *d_pos, int64_t N, i
     if (N == 0) return NF_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     NF_CUDA_OK(c, cudaSetDevice(c->device));
-    nf_status rc = ensure_scratch(c, N);
-    if (rc != NF_OK) return rc;
-    c->last_stream = st; c->lastN = N; c->have_last = 1;
-    rc = nf_run_binner(c, d_pos, N, st);
+    nf_status rc = bin_for(c, d_pos, N, st);
     if (rc != NF_OK) return rc;
     return nf_run_taylor(c, d_pos, order, d_T, d_acc, accumulate ? 1 : 0, st);
 }
@@ -409,6 +486,20 @@ extern "C" nf_status nf_debug_neighbors(nf_ctx *c, int cell, int32_t *h_ids, int
         for (int k = 0; k < 3; ++k) h_image[3 * n + k] = (int8_t)tmp[nn + 3 * n + k];
     }
     free(tmp);
+    return NF_OK;
+}
+
+extern "C" nf_status nf_debug_delivered_pairs(nf_ctx *c, int64_t *h_out) {
+    if (!c || !h_out) return NF_EINVAL;
+    if (!c->have_last || !c->have_sched) { snprintf(c->err, sizeof c->err, "nf_debug_delivered_pairs: the last call on this context was not nf_accel / nf_accel4"); return NF_EINVAL; }
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    NF_CUDA_OK(c, cudaStreamSynchronize(c->last_stream));
+    nf_status rc = nf_run_count(c, c->own_stream);
+    if (rc != NF_OK) return rc;
+    unsigned long long v[2] = {0, 0};
+    NF_CUDA_OK(c, cudaMemcpyAsync(v, c->d_pairs + 6, 16, cudaMemcpyDeviceToHost, c->own_stream));
+    NF_CUDA_OK(c, cudaStreamSynchronize(c->own_stream));
+    h_out[0] = (int64_t)v[0]; h_out[1] = (int64_t)v[1];
     return NF_OK;
 }
 

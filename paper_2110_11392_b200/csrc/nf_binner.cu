@@ -17,17 +17,6 @@
 #include "nf_common.cuh"
 
 // ------------------------------------------------------------------------------ A1
-__device__ __forceinline__ int nf_axis_cell(float x, double scale, int cpd, int &bad) {
-    double xd = (double)x;
-    if (!isfinite(xd)) { bad = 1; return 0; }
-    double t = xd * scale;
-    double I = floor(t);
-    if (I >= 0.0 && I < (double)cpd) return (int)I;
-    double m = fmod(I, (double)cpd);      // exact
-    if (m < 0.0) m += (double)cpd;
-    return (int)m;
-}
-
 __global__ void __launch_bounds__(256) k_key_hist(const float *__restrict__ pos, uint32_t N, double scale, int cpd,
                                                   uint32_t *__restrict__ key, uint32_t *__restrict__ arr,
                                                   uint32_t *__restrict__ counts, uint32_t *__restrict__ ctrl) {

@@ -20,16 +20,10 @@
 #ifndef NF_NW
 #define NF_NW 4                   // consumer warps per CTA
 #endif
-#ifndef NF_PRODUCER_WARP
-#define NF_PRODUCER_WARP 0        // 1: a dedicated producer warp per CTA; 0: consumer warp 0 also fills the ring
-#endif
-#ifndef NF_SHARED_REFILL
-#define NF_SHARED_REFILL 1        // 1 (with NF_PRODUCER_WARP 0): any consumer warp refills the ring, under a lock; 0: warp 0 does
-#endif
 #ifndef NF_REFILL_BELOW
 #define NF_REFILL_BELOW 2          // a warp tries to refill when fewer than this many produced stages lie ahead of it
 #endif
-#define NF_CTA_THREADS ((NF_NW + NF_PRODUCER_WARP) * 32)
+#define NF_CTA_THREADS (NF_NW * 32)
 #ifndef NF_SINKS
 #define NF_SINKS 2                // sinks per consumer thread (adjacent slots 2t, 2t+1 of the warp's range when 2)
 #endif
@@ -49,12 +43,6 @@
 #endif
 #ifndef NF_MIN_CTAS
 #define NF_MIN_CTAS 4             // resident CTAs per SM the interaction kernel is compiled for
-#endif
-#ifndef NF_PRODUCER_SLEEP_NS
-#define NF_PRODUCER_SLEEP_NS 0    // back-off of a dedicated producer warp (NF_PRODUCER_WARP = 1) while its ring slot is in use
-#endif
-#ifndef NF_CONSUMER_SLEEP_NS
-#define NF_CONSUMER_SLEEP_NS 0
 #endif
 
 struct NfParams {
@@ -85,7 +73,7 @@ struct nf_ctx {
     int opt_stage_timing, opt_kahan, opt_heavy_first;
     float opt_rc;                // close-pair radius in cells; < 0 = automatic
     // scratch (grow-only)
-    int64_t capN, capPad, capBlk;
+    int64_t capN, capPad, capBlk, capScan;
     uint32_t *d_key, *d_arr, *d_counts, *d_offsets, *d_poff, *d_tmp_perm, *d_perm_true, *d_perm_pad;
     unsigned long long *d_scan_in, *d_scan_blk;
     float *d_sorted;             // 4 planes of capPad: x, y, z (cell units), cell key (uint32 bits)
@@ -103,6 +91,10 @@ struct nf_ctx {
     cudaStream_t last_stream;
     int64_t lastN;
     int have_last;
+    int bin_pinned;              // nf_bin: the binning of (bin_pos, bin_N) is kept and reused until the particles move
+    const float *bin_pos;
+    int64_t bin_N;
+    int have_sched;              // the sink blocks of the last nf_accel / nf_accel4 are still in d_blk (nf_debug_delivered_pairs)
     int64_t launches;            // kernels launched by this context (nf_launch_count)
     cudaEvent_t ev[8];
     char err[512];
@@ -130,6 +122,10 @@ nf_status nf_run_timestep_ratio(nf_ctx *ctx, const float *d_vel, const float *d_
 nf_status nf_run_taylor(nf_ctx *ctx, const float *d_pos, int order, const double *d_T, float *d_acc, int accumulate, cudaStream_t st);
 nf_status nf_run_f64(nf_ctx *ctx, const float *d_pos, int64_t N, double *d_acc, cudaStream_t st);
 nf_status nf_run_paircount(nf_ctx *ctx, cudaStream_t st);
+nf_status nf_run_count(nf_ctx *ctx, cudaStream_t st);
+nf_status nf_run_cell_histogram(nf_ctx *ctx, const float *d_pos, int64_t N, int32_t *d_counts, cudaStream_t st);
+nf_status nf_run_slab_pairs(nf_ctx *ctx, const int32_t *d_counts, long long *d_pairs, long long *d_npart, cudaStream_t st);
+nf_status nf_run_select_slabs(nf_ctx *ctx, const float *d_pos, int64_t N, int x0, int nx, float *d_out, uint32_t *d_blk, cudaStream_t st);
 nf_status nf_interact_setup(nf_ctx *ctx);
 nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st);
 
@@ -145,4 +141,16 @@ __device__ __forceinline__ int nf_wrap1(int v, int cpd, int &image) {
 __device__ __forceinline__ int nf_mod(int v, int cpd) {
     int m = v % cpd;
     return m < 0 ? m + cpd : m;
+}
+// A1's cell rule for one axis (reading S5): I = floor((double)x * CPD / box), cell = I mod CPD for
+// any finite x (half-open cells, periodic wrap); a NaN/Inf position sets `bad`
+__device__ __forceinline__ int nf_axis_cell(float x, double scale, int cpd, int &bad) {
+    double xd = (double)x;
+    if (!isfinite(xd)) { bad = 1; return 0; }
+    double t = xd * scale;
+    double I = floor(t);
+    if (I >= 0.0 && I < (double)cpd) return (int)I;
+    double m = fmod(I, (double)cpd);      // exact
+    if (m < 0.0) m += (double)cpd;
+    return (int)m;
 }

@@ -4,8 +4,8 @@
 // validating the float32 kernel against a double one.  This is that build as
 // a second entry point: same binning (A1-A3), then a plain tiled direct sum in double --
 // offsets recomputed in double from the caller's float32 positions (not the float32 planes),
-// integer cell shift added last, piecewise Eq. 3 or Eq. 2 with a
-// branch, one accumulator per sink, sources of a cell in ascending input order.  No packed
+// integer cell shift added last, piecewise Eq. 3, Eq. 2 or the
+// unsoftened r/|r|^3 with a branch, one accumulator per sink, sources of a cell in ascending input order.  No packed
 // arithmetic, no clamping, no close-pair path: it is the reference the fast kernel can be held
 // against on EVERY particle of a full-size input (tests/test_gpu_f64.py), where the CPU oracle
 // only reaches samples.  Not on the timed path.
@@ -81,6 +81,8 @@ __global__ void __launch_bounds__(NF64_THREADS) k_direct_f64(const F64Args A) {
                                 if (A.law == NF_SOFT_PLUMMER) {
                                     const double s2 = r2 + A.eps_p * A.eps_p;
                                     f = 1.0 / (s2 * sqrt(s2));
+                                } else if (A.law == NF_SOFT_NEWTON) {
+                                    f = 1.0 / (r2 * sqrt(r2));                  // no softening
                                 } else {
                                     const double r = sqrt(r2);
                                     if (r < A.eps_s) {

@@ -51,13 +51,8 @@ __device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {     
         "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     return ok != 0u;
 }
-// SLEEP_NS > 0: back off between polls so that a waiting warp does not take issue slots from
-// the working warps of its SM sub-partition (the producer is always several stages ahead).
-template <int SLEEP_NS>
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-    while (!mbar_try(bar, parity)) {
-        if (SLEEP_NS > 0) __nanosleep(SLEEP_NS);
-    }
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {     // try_wait suspends in hardware between polls
+    while (!mbar_try(bar, parity)) {}
 }
 __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
@@ -154,7 +149,15 @@ __global__ void __launch_bounds__(256) k_density(int ncell, const uint32_t *__re
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
     if ((threadIdx.x & 31) == 0 && v) atomicAdd(sum2, v);
 }
-__global__ void k_choose_rc(const unsigned long long *__restrict__ sum2, double N, double eps_cells, double soft2, float rc_override,
+// law: NF_SOFT_SPLINE / NF_SOFT_PLUMMER / NF_SOFT_NEWTON.  For the spline the near cells of the
+// close-pair regime evaluate only min(r^-3, r_c^-3) and leave Eq. 3's polynomial to close_scan,
+// so a non-zero r_c must never lie below eps_s: pairs with r_c <= r < eps_s would get r^-3
+// (PAPER.md:132).  Hence r_c, chosen or forced, is raised to eps_s when it falls short of it, and
+// the 0.25-cell cap only applies above eps_s.  Without softening (Newton) there is no core to
+// estimate rms|a| from: the estimate uses the production softening, eps_s = 2.16/40 of the
+// particle-weighted mean spacing, and r_c is kept positive, so that the self pair
+// and coincident pairs meet the finite clamp (f = r_c^-3, d = 0) instead of inf * 0.
+__global__ void k_choose_rc(const unsigned long long *__restrict__ sum2, double N, double eps_cells, double soft2, int law, float rc_override,
                             float *__restrict__ dyn) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     double rc;
@@ -162,20 +165,23 @@ __global__ void k_choose_rc(const unsigned long long *__restrict__ sum2, double 
         rc = rc_override;
     } else {
         const double npw = (double)(*sum2) / N;
-        const double rms = sqrt(4.0 * 3.14159265358979 * npw / eps_cells);
+        const double eps_rms = law == NF_SOFT_NEWTON ? NF_SPLINE_PER_PLUMMER / 40.0 / cbrt(npw) : eps_cells;
+        const double rms = sqrt(4.0 * 3.14159265358979 * npw / eps_rms);
         const double budget = 0.4e-5 * rms;
         rc = 0.05;
         for (int it = 0; it < 20; ++it) rc = sqrt((1.0e-6 + 1.2e-7 / rc) / budget);
-        if (rc < eps_cells) {
+        if (law != NF_SOFT_NEWTON && rc < eps_cells) {
             // inside the core F <= 2.01/eps^2 and |dF/dr| <= 10/eps^3
             const double core = 2.01 / (eps_cells * eps_cells) * 1.0e-6 + 10.0 / (eps_cells * eps_cells * eps_cells) * 6.0e-8;
             rc = (core <= budget) ? 0.0 : eps_cells;
         }
         if (rc > 0.25) rc = 0.25;
     }
+    if (law == NF_SOFT_SPLINE && rc > 0.0 && rc < eps_cells) rc = eps_cells;
+    if (law == NF_SOFT_NEWTON && rc < 1.0e-4) rc = 1.0e-4;
     dyn[0] = (float)(rc * rc);
     dyn[1] = (float)rc;
-    // soft2 = eps_p^2 (cell units) for Plummer softening (the loop's r^2 carries it), 0 for the spline
+    // soft2 = eps_p^2 (cell units) for Plummer softening (the loop's r^2 carries it), 0 otherwise
     const double rs2 = rc * rc + soft2;
     dyn[2] = rc > 0.0 ? (float)(1.0 / (rs2 * sqrt(rs2))) : 0.f;   // clamp of the float32 force factor in near cells
     dyn[3] = (float)rs2;                                           // what the loop's r^2 (+ soft2) is compared with
@@ -189,7 +195,7 @@ nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st) {
     {
         const double ep = ctx->eps_p * ctx->prm.scale;       // eps_p in cell units
         const bool plummer = ctx->law == NF_SOFT_PLUMMER;
-        k_choose_rc<<<1, 32, 0, st>>>(sum2, (double)N, plummer ? ep : ctx->prm.eps_cells, plummer ? ep * ep : 0.0, ctx->opt_rc,
+        k_choose_rc<<<1, 32, 0, st>>>(sum2, (double)N, plummer ? ep : ctx->prm.eps_cells, plummer ? ep * ep : 0.0, ctx->law, ctx->opt_rc,
                                       (float *)(ctx->d_ctrl + 96)); ctx->launches++;
     }
     k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->slab_x0, ctx->slab_nx, ctx->d_poff, ctx->d_col_nblk); ctx->launches++;
@@ -236,7 +242,7 @@ struct __align__(128) Stage {
 struct ProdState {       // cursor of the stage producer (block, column, z-run, chunk), kept in shared memory
     int mode;            // 0 next block, 1 next z-run, 5 z-run requested, 2 next chunk of the run, 3 end of block, 4 finished
     int flags, a, b, u, U1, Z1, ci, cj, ucur, run;
-    int owner;           // warp whose register holds the requested table (NF_SHARED_REFILL)
+    int owner;           // warp whose register holds the requested table
     uint32_t col, s0, cnt, c0, ge;
 };
 
@@ -253,6 +259,8 @@ struct InteractArgs {
     float wfac;              // cell^2: density sum to length units
     int ostride;             // floats per output particle: 3, or 4 with the density estimate in the 4th
     int near_cheb;           // cells within this Chebyshev distance run the near-cell form
+    double close_eps;        // eps_s in cell units for close_scan's Eq. 3 branch (0: no softening, NF_SOFT_NEWTON)
+    unsigned long long *count_out;   // COUNT instantiation: [0] (sink, source) deliveries, [1] deliveries of a sink to itself
     NfParams prm;
 };
 
@@ -337,7 +345,7 @@ __device__ __forceinline__ float fmin3(float a, float b, float c) {
 // MODE 0: far cells, pure r^-3 (11 FMA-pipe ops per pair)
 // MODE 1: near cells, Eq. 3 as min(r^-3, spline) (14 ops)        -- used when no close-pair radius is needed
 // MODE 2: near cells, min(r^-3, r_c^-3) and the running minimum of r^2 (close pairs are fixed up by close_scan)
-// MODE 3: as 2 for the sinks' own cells: the self pair (r^2 == tau exactly, contributes 0) does not count as close
+// MODE 3: as 2 for the sinks' own cells: the self pair (d == 0 exactly, contributes 0) does not count as close
 // Sources [lo, lo + n) of the stage (lo may differ between lanes, n is warp-uniform and a
 // multiple of 4; cells start on 16-byte boundaries) against the NF_SINKS sinks of this thread:
 // four sources per LDS.128 and plane, shared by the thread's sinks.
@@ -356,6 +364,8 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
 #pragma unroll
     for (int j = 0; j < kS; ++j) { nx[j] = make_float2(-xim[j], -xim[j]); ny[j] = make_float2(-yi[j], -yi[j]); nz[j] = make_float2(-zi[j], -zi[j]); }
     float m[kS];
+#pragma unroll
+    for (int j = 0; j < kS; ++j) m[j] = NF_BIG;
     auto pair2 = [&](const int j, const float2 X, const float2 Y, const float2 Z) {
         const float2 dx = __fadd2_rn(X, nx[j]), dy = __fadd2_rn(Y, ny[j]), dz = __fadd2_rn(Z, nz[j]);
         float2 r2 = __ffma2_rn(dx, dx, tau);
@@ -374,8 +384,11 @@ __device__ __forceinline__ void pair_loop(const float *__restrict__ xs, const fl
         if (MODE >= 2) {
             f.x = fminf(f.x, fmax);
             f.y = fminf(f.y, fmax);
-            if (MODE == 2 || LAW != 0) m[j] = fmin3(m[j], r2.x, r2.y);   // Plummer: the self pair is flagged and dropped by close_scan
-            else m[j] = fmin3(m[j], r2.x > 2.f * NF_TAU ? r2.x : NF_BIG, r2.y > 2.f * NF_TAU ? r2.y : NF_BIG);
+            if (MODE == 2) m[j] = fmin3(m[j], r2.x, r2.y);
+            else if (LAW == 0) m[j] = fmin3(m[j], r2.x > 2.f * NF_TAU ? r2.x : NF_BIG, r2.y > 2.f * NF_TAU ? r2.y : NF_BIG);
+            else                                           // Plummer: r^2 carries eps_p^2, so the self pair is told by d == 0 (home cells only)
+                m[j] = fmin3(m[j], (fabsf(dx.x) + fabsf(dy.x) + fabsf(dz.x) > 0.f) ? r2.x : NF_BIG,
+                             (fabsf(dx.y) + fabsf(dy.y) + fabsf(dz.y) > 0.f) ? r2.y : NF_BIG);
         }
         if (DENS && MODE >= 1) {                           // b^2 - r^2 for r < b; the self pair's b^2 is taken off at the end
             const float2 t = __fadd2_rn(b2v, make_float2(-r2.x, -r2.y));
@@ -452,7 +465,10 @@ __device__ __forceinline__ void fold(float &tot, float &comp, float v, int kahan
 // are launched; the one whose regime is not in force returns at once (no host round trip).
 // LAW: NF_SOFT_SPLINE (Eq. 3) or NF_SOFT_PLUMMER (Eq. 2).  DENS: also accumulate the FoF-scale density
 // estimate in the near cells and store it as the 4th output component.
-template <bool FLAG, int LAW, bool DENS>
+// COUNT: a test instantiation (nf_debug_delivered_pairs) that runs the same ring, cursor and passes
+// but, instead of the pair arithmetic, counts the real sources each pass delivers to each real
+// sink: the pair count of what the kernel visited, measured rather than derived from the offsets.
+template <bool FLAG, int LAW, bool DENS, bool COUNT>
 __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const InteractArgs A) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Stage *stages = reinterpret_cast<Stage *>(smem_raw);
@@ -477,109 +493,23 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
     int stage = 0;
     uint32_t phase = 0;
 
-#if NF_PRODUCER_WARP
-    if (warp == NF_NW) {
-        // =========================== producer warp ===========================================
-        const uint32_t nblocks = A.ctrl[1];
-        auto emit = [&](int flags, int a, int b, int zu0, int nc, uint32_t tabval, uint32_t g_lo, int g_cnt, uint32_t col, uint32_t s0, uint32_t cnt) {
-            Stage &S = stages[stage];
-            mbar_wait<NF_PRODUCER_SLEEP_NS>(&empty_bar[stage], phase ^ 1u);
-            S.tab[lane] = tabval;
-            if (lane == 0) {
-                StageHdr h;
-                h.flags = flags; h.a = a; h.b = b; h.zu0 = zu0; h.nc = nc; h.g_lo = g_lo; h.g_cnt = g_cnt;
-                h.col = col; h.s0 = s0; h.cnt = cnt; h.pad0 = 0; h.pad1 = 0;
-                S.hdr = h;
-            }
-            __syncwarp();
-            if (lane == 0) {
-                if (g_cnt > 0) {
-                    const uint32_t bytes = (uint32_t)g_cnt * 4u;
-                    mbar_arrive_expect_tx(&full_bar[stage], 3u * bytes);
-                    bulk_g2s(S.xs, A.sx + g_lo, bytes, &full_bar[stage]);
-                    bulk_g2s(S.ys, A.sy + g_lo, bytes, &full_bar[stage]);
-                    bulk_g2s(S.zs, A.sz + g_lo, bytes, &full_bar[stage]);
-                } else {
-                    mbar_arrive(&full_bar[stage]);
-                }
-            }
-            if (++stage == NF_NSTAGE) { stage = 0; phase ^= 1u; }
-        };
-
-        for (;;) {
-            uint32_t w = 0;
-            if (lane == 0) w = atomicAdd(&A.ctrl[0], 1u);
-            w = __shfl_sync(0xffffffffu, w, 0);
-            if (w >= nblocks) break;
-            const NfBlockDesc d = A.blk[A.order[w]];
-            if (d.cnt == 0) continue;
-            const int ci = (int)(d.col / (uint32_t)cpd), cj = (int)(d.col % (uint32_t)cpd);
-            const int colbase = (int)d.col * cpd;
-            const int Z1 = (int)(A.skey[d.s0] & ~NF_PAD_FLAG) - colbase;
-            const int Z2 = (int)(A.skey[d.s0 + d.cnt - 1] & ~NF_PAD_FLAG) - colbase;
-            int flags = NF_F_NEWBLOCK;
-            for (int a = -R; a <= R; ++a) {
-                int ia; const int sci = nf_wrap1(ci + a, cpd, ia);
-                for (int b = -R; b <= R; ++b) {
-                    int ib; const int scj = nf_wrap1(cj + b, cpd, ib);
-                    const int cb = (sci * cpd + scj) * cpd;
-                    int u = Z1 - R;
-                    const int U1 = Z2 + R;
-                    while (u <= U1) {
-                        const int wz = nf_mod(u, cpd);
-                        int run = U1 - u + 1;
-                        if (run > cpd - wz) run = cpd - wz;
-                        if (run > NF_TABMAX) run = NF_TABMAX;
-                        // table: padded offsets of cells wz .. wz+run (run+1 entries)
-                        const uint32_t tv = A.poff[cb + wz + (lane <= run ? lane : run)];
-                        const uint32_t g0 = __shfl_sync(0xffffffffu, tv, 0);
-                        const uint32_t g1 = __shfl_sync(0xffffffffu, tv, run);
-                        if (g1 > g0) {
-                            const uint32_t gl = g0 & ~3u, ge = (g1 + 3u) & ~3u;
-                            for (uint32_t c0 = gl; c0 < ge; c0 += NF_TILE) {
-                                const uint32_t c1 = (c0 + NF_TILE < ge) ? c0 + NF_TILE : ge;
-                                {
-                                    // table entry = first slot of the cell relative to this stage, clamped to the stage
-                                    int tl = (int)(tv - c0);
-                                    const int tc = (int)(c1 - c0);
-                                    tl = tl < 0 ? 0 : (tl > tc ? tc : tl);
-                                    emit(flags, a, b, u, run, (uint32_t)tl, c0, tc, d.col, d.s0, d.cnt);
-                                }
-                                flags = 0;
-                            }
-                        }
-                        u += run;
-                    }
-                }
-            }
-            emit(flags | NF_F_LAST, 0, 0, 0, 0, 0u, 0u, 0, d.col, d.s0, d.cnt);
-        }
-        emit(NF_F_EXIT, 0, 0, 0, 0, 0u, 0u, 0, 0u, 0u, 0u);
-        return;
-    }
-#else
-    // =========================== production by consumer warp 0 ================================
+    // =========================== stage production by the consumer warps ========================
     // No dedicated producer warp: its registers go to the consumers (4 CTAs x 4 warps x 128
-    // registers fill the register file).  Consumer warps refill freed ring slots at their stage
-    // boundaries (NF_SHARED_REFILL: any warp with little produced work ahead of it, under a lock;
-    // else warp 0); the (block, column, z-run, chunk) cursor lives in shared memory so that it
-    // costs no registers in the pair loop.  produce_one() emits exactly one stage.
+    // registers fill the register file).  A consumer warp that reaches a stage boundary with
+    // fewer than NF_REFILL_BELOW produced stages ahead of it takes a lock and refills freed ring
+    // slots, so the warps that would otherwise wait for data do the production work; the (block,
+    // column, z-run, chunk) cursor lives in shared memory so that it costs no registers in the
+    // pair loop.  produce_one() emits exactly one stage.
     __shared__ ProdState ps;
     __shared__ uint32_t ptab[32];
-#if NF_SHARED_REFILL
-    // Any warp may refill: the one that gets to a stage boundary with room in the ring takes a lock
-    // and emits stages, so the warps that would otherwise wait for data do the production work.
     __shared__ volatile uint32_t nprod_sh;     // stages produced so far
     __shared__ volatile int pdone_sh;          // the EXIT stage has been emitted
     __shared__ int plock;
     uint32_t cons = 0;                         // stages this warp has consumed
-    if (threadIdx.x == 0) { nprod_sh = 0u; pdone_sh = 0; plock = 0; ps.owner = -1; }
-#endif
-    if (threadIdx.x == 0) { ps.mode = 0; ps.flags = 0; }
+    if (threadIdx.x == 0) { nprod_sh = 0u; pdone_sh = 0; plock = 0; ps.owner = -1; ps.mode = 0; ps.flags = 0; }
     __syncthreads();
-    int pstage = 0, ahead = 0;
+    int pstage = 0;
     uint32_t pphase = 0;
-    bool pdone = false;
     uint32_t tvp = 0;        // table entry of the requested run (lane l: padded offset of its cell l), in flight between calls
     // advance the cursor to the next z-run of the block's source columns and request its table
     // (padded offsets of cells wz .. wz+run); mode 5 = requested, mode 3 = the block has no more runs
@@ -645,13 +575,11 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
             }
             if (q.mode == 1) issue_run(q);           // (only right after a block start or an empty run: not prefetched)
             if (q.mode == 5) {                       // the run's table has been requested: is the run non-empty?
-#if NF_SHARED_REFILL
                 if (q.owner != warp) {               // requested by another warp: fetch it again (cache-hot by now)
                     int ia; const int sci = nf_wrap1(q.ci + q.a, cpd, ia);
                     int ib; const int scj = nf_wrap1(q.cj + q.b, cpd, ib);
                     tvp = A.poff[(sci * cpd + scj) * cpd + nf_mod(q.ucur, cpd) + (lane <= q.run ? lane : q.run)];
                 }
-#endif
                 const uint32_t g0 = __shfl_sync(0xffffffffu, tvp, 0);
                 const uint32_t g1 = __shfl_sync(0xffffffffu, tvp, q.run);
                 if (g1 <= g0) { q.mode = 1; continue; }
@@ -683,8 +611,6 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
         return last;
     };
 
-#endif
-
     // =============================== consumer warps ==========================================
     // Thread t of warp w holds the kS sinks at slots s0 + (32 w + t) kS + j of the block (adjacent
     // slots: cells are padded to 4 slots and blocks start on multiples of 4, so they share a cell).
@@ -693,7 +619,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
     const float rc2 = A.dyn[3];
     const float fmax = A.dyn[2];
     CloseArgs K;
-    K.pos = A.pos; K.perm_pad = A.perm_pad; K.scale = A.prm.scale; K.eps = A.prm.eps_cells;
+    K.pos = A.pos; K.perm_pad = A.perm_pad; K.scale = A.prm.scale; K.eps = A.close_eps;
     K.law = LAW; K.addend = A.addend; K.soft2 = (LAW == NF_SOFT_PLUMMER) ? (double)A.addend : 0.0;
     const int tid_s = (int)threadIdx.x * kS;           // this thread's first column of close_corr / tot
     float px[kS], py[kS], pz[kS];
@@ -703,10 +629,9 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
     bool valid = false;
     uint32_t slot = 0;
     const int W = 2 * R + 1;
+    unsigned long long n_deliv = 0ull, n_self = 0ull;   // COUNT only
 
     for (;;) {
-#if !NF_PRODUCER_WARP
-#if NF_SHARED_REFILL
         while (!pdone_sh) {
             uint32_t np = nprod_sh;
             np = __shfl_sync(0xffffffffu, np, 0);
@@ -723,7 +648,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                 pstage = (int)(np % NF_NSTAGE);
                 pphase = (np / NF_NSTAGE) & 1u;
                 bool ok = mbar_test(&empty_bar[pstage], pphase ^ 1u);
-                if (!ok && np == cons) { mbar_wait<0>(&empty_bar[pstage], pphase ^ 1u); ok = true; }   // starved: wait for the slot
+                if (!ok && np == cons) { mbar_wait(&empty_bar[pstage], pphase ^ 1u); ok = true; }   // starved: wait for the slot
                 if (ok) {
                     const bool last = produce_one();
                     if (lane == 0) { if (last) pdone_sh = 1; __threadfence_block(); nprod_sh = np + 1u; }
@@ -738,22 +663,8 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
             __syncwarp();
             if (released) break;
         }
-#else
-        if (warp == 0 && !pdone) {
-            // refill every free slot; block only when there is nothing left to consume
-            while (ahead < NF_NSTAGE) {
-                if (ahead > 0) { if (!mbar_test(&empty_bar[pstage], pphase ^ 1u)) break; }
-                else mbar_wait<0>(&empty_bar[pstage], pphase ^ 1u);
-                pdone = produce_one();
-                if (++pstage == NF_NSTAGE) { pstage = 0; pphase ^= 1u; }
-                ++ahead;
-                if (pdone) break;
-            }
-        }
-#endif
-#endif
         Stage &S = stages[stage];
-        mbar_wait<NF_CONSUMER_SLEEP_NS>(&full_bar[stage], phase);
+        mbar_wait(&full_bar[stage], phase);
         const int flags = S.hdr.flags;
         if (flags & NF_F_EXIT) break;
         if (flags & NF_F_NEWBLOCK) {
@@ -808,11 +719,6 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
             // it is masked.  cB = cA + 2R+1, so the two lane groups are disjoint: the edge cells
             // of the warp's window, each needed by only part of the warp, are processed two at a
             // time and no lane idles.
-            // One pass = sources [lo, lo + n) where a lane reads cell cA's part (from loA) if its
-            // sink is within R cells of cA, else cell cB's part (from loB) if within R of cB, else
-            // it is masked.  cB = cA + 2R+1, so the two lane groups are disjoint: the edge cells
-            // of the warp's window, each needed by only part of the warp, are processed two at a
-            // time and no lane idles.
             auto pass = [&](const int ploA, const int pcA, const int ploB, const int pcB, const int n, const int mode) __attribute__((always_inline)) {
                 const bool useA = abs(zl - pcA) <= R, useB = abs(zl - pcB) <= R;
                 const int cell = useA ? pcA : pcB;
@@ -825,6 +731,18 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                     xim[j] = (useA || useB) ? xi[j] : -NF_BIG;    // masked sink at -BIG, padding sources at +BIG: never coincide
                     zi[j] = pz[j] - (float)dzc;
                     bits[j] = 0u;
+                }
+                if (COUNT) {
+                    uint32_t nreal = 0;
+                    for (int s = lo; s < lo + n; ++s) nreal += S.xs[s] < 0.5f * NF_BIG ? 1u : 0u;
+#pragma unroll
+                    for (int j = 0; j < kS; ++j)
+                        if ((useA || useB) && valid && fabsf(px[j]) < 0.5f * NF_BIG) {      // a real sink that this pass serves
+                            n_deliv += nreal;
+                            const uint32_t rel = slot + j - S.hdr.g_lo;                    // the sink's own slot, stage-local
+                            if (rel >= (uint32_t)lo && rel < (uint32_t)(lo + n) && dzc == 0 && ha == 0 && hb == 0) n_self += 1ull;
+                        }
+                    return;
                 }
                 if (mode == 0) pair_loop<0, false, LAW, DENS>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits, A.addend, A.b2, aw);
                 else if (!FLAG) pair_loop<1, false, LAW, DENS>(S.xs, S.ys, S.zs, lo, n, xim, yi, zi, ax, ay, az, c0, c1, c2, fmax, rc2, 0, bits, A.addend, A.b2, aw);
@@ -880,7 +798,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                 if (DENS) tot[DENS ? 6 : 0][tid_s + j] += aw[j].x + aw[j].y;
             }
         }
-        if (flags & NF_F_LAST) {
+        if ((flags & NF_F_LAST) && !COUNT) {
             if (valid) {
 #pragma unroll
                 for (int j = 0; j < kS; ++j) {
@@ -899,13 +817,12 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty_bar[stage]);
         if (++stage == NF_NSTAGE) { stage = 0; phase ^= 1u; }
-#if !NF_PRODUCER_WARP
-#if NF_SHARED_REFILL
         ++cons;
-#else
-        --ahead;
-#endif
-#endif
+    }
+    if (COUNT) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) { n_deliv += __shfl_xor_sync(0xffffffffu, n_deliv, d); n_self += __shfl_xor_sync(0xffffffffu, n_self, d); }
+        if (lane == 0) { atomicAdd(A.count_out, n_deliv); atomicAdd(A.count_out + 1, n_self); }
     }
 }
 
@@ -915,11 +832,14 @@ typedef void (*InteractKernel)(const InteractArgs);
 // [law][dens][flag]
 static InteractKernel interact_kernel(int law, int dens, int flag) {
     static const InteractKernel tab[2][2][2] = {
-        {{k_interact<false, NF_SOFT_SPLINE, false>, k_interact<true, NF_SOFT_SPLINE, false>},
-         {k_interact<false, NF_SOFT_SPLINE, true>, k_interact<true, NF_SOFT_SPLINE, true>}},
-        {{k_interact<false, NF_SOFT_PLUMMER, false>, k_interact<true, NF_SOFT_PLUMMER, false>},
-         {k_interact<false, NF_SOFT_PLUMMER, true>, k_interact<true, NF_SOFT_PLUMMER, true>}}};
+        {{k_interact<false, NF_SOFT_SPLINE, false, false>, k_interact<true, NF_SOFT_SPLINE, false, false>},
+         {k_interact<false, NF_SOFT_SPLINE, true, false>, k_interact<true, NF_SOFT_SPLINE, true, false>}},
+        {{k_interact<false, NF_SOFT_PLUMMER, false, false>, k_interact<true, NF_SOFT_PLUMMER, false, false>},
+         {k_interact<false, NF_SOFT_PLUMMER, true, false>, k_interact<true, NF_SOFT_PLUMMER, true, false>}}};
     return tab[law][dens][flag];
+}
+static InteractKernel count_kernel(int flag) {
+    return flag ? k_interact<true, NF_SOFT_SPLINE, false, true> : k_interact<false, NF_SOFT_SPLINE, false, true>;
 }
 
 nf_status nf_interact_setup(nf_ctx *ctx) {
@@ -934,14 +854,13 @@ nf_status nf_interact_setup(nf_ctx *ctx) {
                 NF_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n1, k, NF_CTA_THREADS, smem));
                 if (n1 < nb) nb = n1;
             }
+    for (int flag = 0; flag < 2; ++flag) NF_CUDA_OK(ctx, cudaFuncSetAttribute(count_kernel(flag), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (nb < 1) { snprintf(ctx->err, sizeof(ctx->err), "interaction kernel does not fit on an SM"); return NF_ECUDA; }
     g_interact_blocks_per_sm = nb;
     return NF_OK;
 }
 
-// d_out: N x ostride floats (ostride 3: accelerations; 4: accelerations + density estimate, PAPER.md:256)
-nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st) {
-    InteractArgs A;
+static void fill_interact_args(nf_ctx *ctx, const float *d_pos, float *d_out, int ostride, float kfac, InteractArgs &A, int &law, int &dens) {
     A.pos = d_pos;
     A.sx = ctx->d_sorted; A.sy = ctx->d_sorted + ctx->capPad; A.sz = ctx->d_sorted + 2ull * ctx->capPad;
     A.skey = (const uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
@@ -949,22 +868,48 @@ nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_o
     A.ctrl = ctx->d_ctrl; A.dyn = (const float *)(ctx->d_ctrl + 96); A.acc = d_out; A.kfac = kfac; A.prm = ctx->prm;
     A.prm.kahan = ctx->opt_kahan;
     A.ostride = ostride;
-    const int law = ctx->law == NF_SOFT_PLUMMER ? 1 : 0;
-    const int dens = (ostride == 4 && ctx->dens_b > 0.0) ? 1 : 0;
+    A.count_out = ctx->d_pairs + 6;
+    // the unsoftened law runs the spline instantiation in its close-pair regime (k_choose_rc keeps
+    // r_c > 0 for it): r^-3 clamped at r_c^-3 in the near cells, exact 1/r^2 from close_scan below r_c
+    law = ctx->law == NF_SOFT_PLUMMER ? 1 : 0;
+    dens = (ostride == 4 && ctx->dens_b > 0.0) ? 1 : 0;
     const double ep = ctx->eps_p * ctx->prm.scale;            // eps_p in cell units
     A.addend = law ? (float)(ep * ep) : NF_TAU;
+    A.close_eps = ctx->law == NF_SOFT_NEWTON ? 0.0 : ctx->prm.eps_cells;
     const double bc = ctx->dens_b * ctx->prm.scale;           // density radius in cell units
     A.b2 = (float)(bc * bc) + A.addend;
     const double cellsz = ctx->box / (double)ctx->cpd;
     A.wfac = (float)(cellsz * cellsz);
-    // near cells: may hold r < eps_s (spline), or r < b (density)
-    int nc = law ? 1 : ctx->prm.near_cheb;
+    // near cells: may hold r < eps_s (spline), r < r_c <= 0.25 (Plummer, Newton), or r < b (density)
+    int nc = ctx->law == NF_SOFT_SPLINE ? ctx->prm.near_cheb : 1;
     if (dens) { const int nb = (int)ceil(bc); if (nb > nc) nc = nb; }
     if (nc > ctx->R) nc = ctx->R;
     A.near_cheb = nc;
+}
+
+// d_out: N x ostride floats (ostride 3: accelerations; 4: accelerations + density estimate, PAPER.md:256)
+nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st) {
+    InteractArgs A;
+    int law, dens;
+    fill_interact_args(ctx, d_pos, d_out, ostride, kfac, A, law, dens);
     const int grid = ctx->sm_count * g_interact_blocks_per_sm;
     for (int flag = 1; flag >= 0; --flag) {     // the instantiation whose regime is not in force returns at once
         interact_kernel(law, dens, flag)<<<grid, NF_CTA_THREADS, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
+    }
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
+
+// nf_debug_delivered_pairs: the COUNT instantiation over the sink blocks of the last nf_accel
+nf_status nf_run_count(nf_ctx *ctx, cudaStream_t st) {
+    InteractArgs A;
+    int law, dens;
+    fill_interact_args(ctx, nullptr, nullptr, 3, 0.f, A, law, dens);
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_ctrl, 0, sizeof(uint32_t), st));             // the work counter
+    NF_CUDA_OK(ctx, cudaMemsetAsync(A.count_out, 0, 2 * sizeof(unsigned long long), st));
+    const int grid = ctx->sm_count * g_interact_blocks_per_sm;
+    for (int flag = 1; flag >= 0; --flag) {
+        count_kernel(flag)<<<grid, NF_CTA_THREADS, sizeof(Stage) * NF_NSTAGE, st>>>(A); ctx->launches++;
     }
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;

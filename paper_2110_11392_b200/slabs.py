@@ -5,51 +5,29 @@ decomposition", sec. 4.4) and the near field of a slab needs th
 either side (near-field radius, Table 1).  Here: one process per GPU, each rank
 owns a contiguous periodic range of x slabs balanced by PAIR COUNT (not slab count), receives
 the particles of the R ghost slabs on each side from their owners (one point-to-point exchange,
-``torch.distributed`` isend/irecv: NCCL between GPUs, gloo in the CPU tests), and calls
-``nf_accel`` with ``nf_set_sink_slabs`` so that only its own slabs are sinks.  Every sink is owned
-by exactly one rank, so there is no reduction.
+``torch.distributed`` isend/irecv: NCCL between GPUs, gloo in the CPU tests) straight into the
+tail of its own+ghost buffer, and calls ``nf_accel`` with ``nf_set_sink_slabs`` so that only its
+own slabs are sinks.  Every sink is owned by exactly one rank, so there is no reduction.
 
-Everything here is host-side plumbing (index arithmetic, message sizes, send/recv); the force
-arithmetic stays in the CUDA library.  ``slab_index`` repeats the library's cell rule
-(reading S5: floor((double)x * CPD / box) mod CPD) because the owner of a particle
-must be known before it is sent.
+Everything here is host-side plumbing: slab index arithmetic, message sizes, send/recv.  The
+method's arithmetic stays in the CUDA library: which cell a particle is in (``nf_cell_histogram``,
+``nf_select_slabs`` -- step A1's rule), the pair count per slab (``nf_slab_pairs`` -- identity P7)
+and the forces.  The functions that need particles take a ``select(x0, nx) -> tensor`` callable for
+that reason: ``SlabNearField`` passes the library's; the CPU tests of the plumbing pass their own.
 """
 from __future__ import annotations
+
+from typing import Callable
 
 import torch
 
 
-# ----------------------------------------------------------------------------- planning
-def slab_index(pos: torch.Tensor, cpd: int, box: float = 1.0) -> torch.Tensor:
-    """x cell index of every particle (int64, same device): floor((double)x * CPD / box) mod CPD."""
-    t = pos[:, 0].to(torch.float64) * (float(cpd) / float(box))
-    return torch.remainder(torch.floor(t).to(torch.int64), cpd)
-
-
-def cell_index(pos: torch.Tensor, cpd: int, box: float = 1.0) -> torch.Tensor:
-    t = torch.floor(pos.to(torch.float64) * (float(cpd) / float(box))).to(torch.int64)
-    c = torch.remainder(t, cpd)
-    return (c[:, 0] * cpd + c[:, 1]) * cpd + c[:, 2]
-
-
-def pairs_per_slab(counts: torch.Tensor, cpd: int, R: int) -> torch.Tensor:
-    """counts: occupancy histogram [cpd^3] (key = (cx*cpd+cy)*cpd+cz).  Returns, per x slab, the
-    number of (sink, source) pairs whose sink lies in the slab: sum_c n_c (B*n)_c with B the
-    periodic (2R+1)^3 box filter (the integer identity P7 of DESIGN.md), int64 [cpd]."""
-    n = counts.to(torch.int64).reshape(cpd, cpd, cpd)
-    f = n
-    for dim in range(3):
-        acc = torch.zeros_like(f)
-        for s in range(-R, R + 1):
-            acc += torch.roll(f, shifts=s, dims=dim)
-        f = acc
-    return (n * f).sum(dim=(1, 2))
-
-
-def balance_slabs(work: torch.Tensor, world: int) -> list[tuple[int, int]]:
+# ----------------------------------------------------------------------------- planning (integers only)
+def balance_slabs(work, world: int) -> list[tuple[int, int]]:
     """Cut the cpd slabs into ``world`` contiguous ranges [(x0, nx)] of nearly equal work, each
-    with at least one slab (cut k goes where the prefix sum first reaches k/world of the total)."""
-    w = [int(v) for v in work.tolist()]
+    with at least one slab (cut k goes where the prefix sum first reaches k/world of the total).
+    ``work``: per-slab work (``nf_slab_pairs``), any sequence or 1-D tensor of integers."""
+    w = [int(v) for v in (work.tolist() if hasattr(work, "tolist") else work)]
     cpd = len(w)
     if world > cpd:
         raise ValueError(f"{world} ranks need at least {world} slabs, the grid has {cpd}")
@@ -102,85 +80,139 @@ def send_plan(bounds: list[tuple[int, int]], cpd: int, R: int, rank: int) -> dic
     return plan
 
 
+def slab_runs(slabs: list[int], cpd: int) -> list[tuple[int, int]]:
+    """a set of slab indices as periodic runs [(x0, nx)] (a halo is one or two of them)"""
+    left = sorted(set(slabs))
+    runs: list[tuple[int, int]] = []
+    while left:
+        s = set(left)
+        x0 = next((x for x in left if (x - 1) % cpd not in s), left[0])     # a run start (any slab if the set is a full circle)
+        n = 1
+        while (x0 + n) % cpd in s and n < len(s):
+            n += 1
+        runs.append((x0, n))
+        gone = {(x0 + i) % cpd for i in range(n)}
+        left = [x for x in left if x not in gone]
+    return runs
+
+
 # ----------------------------------------------------------------------------- exchange
-def halo_exchange(pos_own: torch.Tensor, xslab_own: torch.Tensor, bounds: list[tuple[int, int]], cpd: int, R: int,
-                  group=None) -> torch.Tensor:
-    """Send the particles of my boundary slabs to the ranks that need them and return the ghost
-    particles I receive ([n_ghost, 3], same dtype/device as pos_own).  One count exchange
-    (all_gather of a [world] vector) and one batch of isend/irecv."""
+Select = Callable[[int, int], torch.Tensor]     # (x0, nx) -> the local particles in x slabs [x0, x0+nx), [n,3]
+
+
+def halo_exchange(select: Select, like: torch.Tensor, bounds: list[tuple[int, int]], cpd: int, R: int, group=None,
+                  recv_into: Callable[[int], torch.Tensor] | None = None) -> torch.Tensor:
+    """Send the particles of my boundary slabs to the ranks that need them and receive my ghosts.
+    One count exchange (all_gather of a [world] vector) and one batch of isend/irecv.
+    ``like``: any tensor of the particles' dtype/device.  ``recv_into(n)``: a contiguous [n,3] view
+    to receive the n ghosts into (the tail of the caller's own+ghost buffer); default: a new tensor.
+    Returns that view."""
     import torch.distributed as dist
+    if not dist.is_initialized() or dist.get_world_size(group) == 1:
+        return like.new_zeros((0, 3))
     world = dist.get_world_size(group)
     rank = dist.get_rank(group)
-    if world == 1:
-        return pos_own.new_zeros((0, 3))
-    plan = send_plan(bounds, cpd, R, rank)
     out = {}
-    counts = torch.zeros(world, dtype=torch.int64, device=pos_own.device)
-    for q, slabs in plan.items():
-        m = torch.zeros(cpd, dtype=torch.bool, device=pos_own.device)
-        m[torch.tensor(slabs, device=pos_own.device)] = True
-        out[q] = pos_own[m[xslab_own]].contiguous()
+    counts = torch.zeros(world, dtype=torch.int64, device=like.device)
+    for q, need in send_plan(bounds, cpd, R, rank).items():
+        parts = [select(x0, nx) for x0, nx in slab_runs(need, cpd)]
+        out[q] = parts[0] if len(parts) == 1 else torch.cat(parts, dim=0)
         counts[q] = out[q].shape[0]
     allc = [torch.zeros_like(counts) for _ in range(world)]
     dist.all_gather(allc, counts, group=group)
-    ops, recv = [], {}
-    for q in range(world):
-        if q == rank:
-            continue
-        nrecv = int(allc[q][rank])
-        if nrecv:
-            recv[q] = pos_own.new_empty((nrecv, 3))
-            ops.append(dist.P2POp(dist.irecv, recv[q], dist.get_global_rank(group, q) if group is not None else q, group))
+    nrecv = {q: int(allc[q][rank]) for q in range(world) if q != rank}
+    total = sum(nrecv.values())
+    ghosts = recv_into(total) if recv_into is not None else like.new_empty((total, 3))
+    peer = (lambda q: dist.get_global_rank(group, q)) if group is not None else (lambda q: q)
+    ops, at = [], 0
+    for q in sorted(nrecv):
+        if nrecv[q]:
+            ops.append(dist.P2POp(dist.irecv, ghosts[at:at + nrecv[q]], peer(q), group))
+            at += nrecv[q]
         if q in out and out[q].shape[0]:
-            ops.append(dist.P2POp(dist.isend, out[q], dist.get_global_rank(group, q) if group is not None else q, group))
+            ops.append(dist.P2POp(dist.isend, out[q], peer(q), group))
     if ops:
         for req in dist.batch_isend_irecv(ops):
             req.wait()
-    if not recv:
-        return pos_own.new_zeros((0, 3))
-    return torch.cat([recv[q] for q in sorted(recv)], dim=0)
+    return ghosts
 
 
-def local_with_ghosts(pos_all: torch.Tensor, bounds: list[tuple[int, int]], cpd: int, R: int, rank: int, box: float = 1.0):
-    """No-communication form for a rank that can see every particle (tests, single-GPU emulation
-    of a decomposition): -> (pos_own, pos_ghost) of ``rank``."""
-    xs = slab_index(pos_all, cpd, box)
+def local_with_ghosts(select: Select, bounds: list[tuple[int, int]], cpd: int, R: int, rank: int):
+    """No-communication form for a process that can see every particle (tests, single-GPU emulation
+    of a decomposition): -> (pos_own, pos_ghost) of ``rank`` from a ``select`` over ALL particles."""
     x0, nx = bounds[rank]
-    own = torch.remainder(xs - x0, cpd) < nx
-    ghost_slabs = halo_slabs(bounds, cpd, R, rank)
-    g = torch.zeros(cpd, dtype=torch.bool, device=pos_all.device)
-    if ghost_slabs:
-        g[torch.tensor(ghost_slabs, device=pos_all.device)] = True
-    return pos_all[own], pos_all[g[xs] & ~own]
+    own = select(x0, nx)
+    runs = slab_runs(halo_slabs(bounds, cpd, R, rank), cpd)
+    parts = [select(a, n) for a, n in runs]
+    ghost = torch.cat(parts, dim=0) if parts else own.new_zeros((0, 3))
+    return own, ghost
 
 
 # ----------------------------------------------------------------------------- the sharded call
+def plan_slabs(nf, pos_own: torch.Tensor, world: int, group=None) -> list[tuple[int, int]]:
+    """pair-balanced slab ranges from the ranks' particles: local histogram (``nf_cell_histogram``),
+    one all_reduce of cpd^3 int32, pairs per slab (``nf_slab_pairs``), cuts on the host."""
+    import torch.distributed as dist
+    counts = nf.cell_histogram(pos_own)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(counts, group=group)
+    pairs, _ = nf.slab_pairs(counts)
+    return balance_slabs(pairs.cpu(), world)
+
+
 class SlabNearField:
     """nf_accel over a slab decomposition: ``accel(pos_own)`` -> accelerations of the rank's own
-    particles.  ``bounds`` = [(x0, nx)] per rank (``balance_slabs``); every particle of
-    ``pos_own`` must lie in the rank's slabs."""
+    particles.  ``bounds`` = [(x0, nx)] per rank (``plan_slabs`` / ``balance_slabs``); every particle
+    of ``pos_own`` must lie in the rank's slabs (``validate=True`` checks it on the device).
+    ``gm`` = G*m of the WHOLE particle set (1/N_global for the paper's unit total mass): the default
+    of the single-GPU call, 1/N of the call, would be 1/(own + ghost) here and differ between ranks."""
 
-    def __init__(self, cpd: int, R: int, eps_plummer: float, box: float, bounds, group=None):
+    def __init__(self, cpd: int, R: int, eps_plummer: float, box: float, bounds, gm: float, group=None):
         import torch.distributed as dist
         from .binding import NearField
         self.cpd, self.R, self.box, self.bounds, self.group = cpd, R, box, list(bounds), group
         self.rank = dist.get_rank(group) if dist.is_initialized() else 0
         self.nf = NearField(cpd, R, eps_plummer, box)
+        self.nf.set_gm(gm)
         x0, nx = self.bounds[self.rank]
         self.nf.set_sink_slabs(x0, nx)
         self.n_ghost = 0
+        self.halo_bytes = 0          # bytes received in the last exchange
+        self._buf = self._acc = self._send = None
 
-    def accel(self, pos_own: torch.Tensor, stream=None) -> torch.Tensor:
-        xs = slab_index(pos_own, self.cpd, self.box)
+    def _room(self, like: torch.Tensor, n: int):
+        if self._buf is None or self._buf.shape[0] < n:
+            cap = int(n * 1.05) + 1024
+            old = self._buf
+            self._buf = like.new_empty((cap, 3))
+            self._acc = like.new_zeros((cap, 3))
+            if old is not None:
+                self._buf[: old.shape[0]] = old
+
+    def accel(self, pos_own: torch.Tensor, stream=None, validate: bool = False) -> torch.Tensor:
+        n_own = pos_own.shape[0]
         x0, nx = self.bounds[self.rank]
-        if not bool((torch.remainder(xs - x0, self.cpd) < nx).all()):
+        if validate and self.nf.select_slabs(pos_own, x0, nx) != n_own:
             raise ValueError("pos_own holds particles outside this rank's slabs")
-        ghosts = halo_exchange(pos_own, xs, self.bounds, self.cpd, self.R, self.group)
+        if self._send is None or self._send.shape[0] < n_own:
+            self._send = pos_own.new_empty((n_own, 3))
+        self._room(pos_own, n_own + max(self.n_ghost, n_own // 8))
+        self._buf[:n_own].copy_(pos_own)
+
+        def select(a, n):
+            k = self.nf.select_slabs(pos_own, a, n, out=self._send)
+            return self._send[:k].clone()
+
+        def recv_into(n):
+            self._room(pos_own, n_own + n)
+            return self._buf[n_own:n_own + n]
+
+        ghosts = halo_exchange(select, pos_own, self.bounds, self.cpd, self.R, self.group, recv_into)
         self.n_ghost = int(ghosts.shape[0])
-        allp = torch.cat([pos_own, ghosts], dim=0).contiguous()
-        acc = torch.zeros_like(allp)
-        self.nf.accel(allp, acc, stream=stream)
-        return acc[: pos_own.shape[0]]
+        self.halo_bytes = self.n_ghost * 12
+        n_tot = n_own + self.n_ghost
+        self.nf.accel(self._buf[:n_tot], self._acc[:n_tot], stream=stream)      # ghost rows of acc are not written
+        return self._acc[:n_own]
 
     def interaction_count(self) -> int:
         return self.nf.interaction_count()

@@ -101,3 +101,63 @@ def test_leapfrog_step_with_the_near_field(torch_cuda, NF, oracle_mod):
     assert d.max() <= 2e-7
     vr = np.sqrt((v2.astype(np.float64) ** 2).sum(1).mean())
     assert np.abs(gv - v2).max() <= 2e-5 * vr
+
+
+def test_bin_once_reuse_everywhere(torch_cuda, NF, oracle_mod):
+    """nf_bin pins the grid order of a position buffer: the force, f64, multipole, Taylor and
+    time-step calls of one step then reuse it (no re-sort: fewer launches, stage times of A1-A3
+    read 0) with bit-identical results; moving the particles (nf_kick_drift) or passing another
+    buffer drops the pin."""
+    torch = torch_cuda
+    cfg = W.scaled(W.CONFIGS[3], 10)
+    pos, vel, acc_in = _state(cfg, 5)
+    d_pos, d_vel = torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda()
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        nf.set_option("stage_timing", 1)
+        n0 = nf.launch_count()
+        a_plain = nf.accel(d_pos).clone()
+        plain_launches = nf.launch_count() - n0
+        M_plain = nf.multipoles(d_pos, 4).clone()
+        f_plain = nf.accel_f64(d_pos).clone()
+        t_plain = nf.timestep_ratio(d_pos, d_vel, a_plain)
+        nf.bin(d_pos)
+        n1 = nf.launch_count()
+        a_pin = nf.accel(d_pos).clone()
+        pinned_launches = nf.launch_count() - n1
+        st = nf.stage_ms()
+        assert pinned_launches <= plain_launches - 6          # key_hist, 3 scans, scatter, rank_gather not launched
+        assert st["A1_key_hist"] == 0.0 and st["A3_scatter_rank_gather"] == 0.0 and st["A5_interact_A6_unpermute"] > 0
+        n2 = nf.launch_count()
+        M_pin = nf.multipoles(d_pos, 4)
+        assert nf.launch_count() - n2 == 1
+        f_pin = nf.accel_f64(d_pos)
+        T = torch.randn_like(M_pin)
+        y_pin = nf.taylor_accel(d_pos, T, 4).clone()
+        t_pin = nf.timestep_ratio(d_pos, d_vel, a_plain)
+        dbg = nf.debug_cells()
+        nf.sync()
+        assert torch.equal(a_pin, a_plain) and torch.equal(M_pin, M_plain) and torch.equal(f_pin, f_plain)
+        assert np.array_equal(t_pin, t_plain)
+        cell, _ = oracle_mod.bin_particles(pos, cfg.cpd)
+        offsets, order = oracle_mod.cell_lists(cell, cfg.cpd)
+        assert np.array_equal(dbg["offsets"].astype(np.int64), offsets) and np.array_equal(dbg["perm"].astype(np.int64), order)
+        # another buffer: sorted as usual, and the pin is gone
+        other = torch.from_numpy(W.uniform(3000, 9)).cuda()
+        b0 = nf.accel(other).clone()
+        n3 = nf.launch_count()
+        nf.accel(d_pos)
+        assert nf.launch_count() - n3 == plain_launches
+        # pinned again, then the particles move: the next call sorts the new positions
+        nf.bin(d_pos)
+        nf.kick_drift(d_pos, d_vel, a_plain, 0.0, 0.05)
+        a_moved = nf.accel(d_pos)
+        y_unpinned = nf.taylor_accel(torch.from_numpy(pos).cuda(), T, 4)
+        nf.sync()
+        moved = d_pos.cpu().numpy()
+        assert torch.equal(y_unpinned, y_pin)
+    ref, _ = oracle_mod.accel(moved, cfg.cpd, cfg.R, cfg.eps_p)
+    g = a_moved.cpu().numpy().astype(np.float64)
+    rms = np.sqrt((ref ** 2).sum(1).mean())
+    assert np.linalg.norm(g - ref, axis=1).max() <= 1e-5 * rms
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf2:
+        assert torch.equal(nf2.accel(other), b0)

@@ -1,5 +1,6 @@
 """Parity of the kernel variants (C ABI: nf_set_softening, nf_set_density_radius, nf_accel4)
-against ``oracle.accel_variant`` on the same seeded inputs.
+against ``oracle.accel_variant`` on the same seeded inputs: Plummer softening (Eq. 2), no softening
+(PAPER.md:218), the FoF-scale density estimate.
 
 Bars: accelerations as in tests/test_gpu_parity.py (north_star: per particle |da| <= 1e-5 rms|a|,
 median relative error <= 2e-6).  Density estimate: a float32 sum of at most a few
@@ -85,9 +86,47 @@ def test_plummer_softening(torch_cuda, NF, oracle_mod, label, cfg):
     got, _, rc = run(torch_cuda, NF, pos, cfg, law="plummer")
     ref, _, _ = oracle_mod.accel_variant(pos, cfg.cpd, cfg.R, cfg.eps_p, law="plummer")
     check_acc(got, ref, f"plummer {label} (rc={rc:.3g})")
+    if rc == 0:                                    # also through the close-pair regime (self pairs told by d == 0)
+        got2, _, rc2 = run(torch_cuda, NF, pos, cfg, law="plummer", opts={"rc_cells": 0.05})
+        assert rc2 > 0
+        check_acc(got2, ref, f"plummer {label} (forced rc={rc2:.3g})")
     # and it is not the spline: the two laws differ where particles are closer than a few eps
     spl, _ = oracle_mod.accel(pos, cfg.cpd, cfg.R, cfg.eps_p)
     assert np.abs(spl - ref).max() > 1e-4 * np.sqrt((ref ** 2).sum(1).mean())
+
+
+@pytest.mark.parametrize("label,cfg", CASES, ids=[c[0] for c in CASES])
+def test_unsoftened_newtonian_law(torch_cuda, NF, oracle_mod, label, cfg):
+    """NF_SOFT_NEWTON (PAPER.md:218 "Newtonian gravity, or a softened form thereof"): r/|r|^3 for every
+    pair, the closest ones through the double-precision close-pair path; eps_p does not enter."""
+    pos = W.make_positions(cfg)
+    got, _, rc = run(torch_cuda, NF, pos, cfg, law="newton")
+    ref, _, _ = oracle_mod.accel_variant(pos, cfg.cpd, cfg.R, cfg.eps_p, law="newton")
+    assert rc > 0
+    check_acc(got, ref, f"newton {label} (rc={rc:.3g})")
+    got0, _, rc0 = run(torch_cuda, NF, pos, cfg, law="newton", opts={"rc_cells": 0.0})      # asked for none: kept at the floor
+    assert 0 < rc0 <= 1.01e-4 and np.isfinite(got0).all()
+    # the f64 entry point follows the same law
+    with NF(cfg.cpd, cfg.R, cfg.eps_p * 7.0, 1.0) as nf:                                     # another eps: ignored
+        nf.set_softening("newton")
+        a64 = nf.accel_f64(torch_cuda.from_numpy(pos).cuda())
+        nf.sync()
+        a64 = a64.cpu().numpy()
+    assert np.abs(a64 - ref).max() <= 1e-12 * np.sqrt((ref ** 2).sum(1).mean())
+
+
+def test_newton_two_particles_and_coincident(torch_cuda, NF, oracle_mod):
+    cfg = W.Config("n2", 8, 2, 0, "uniform", 0.01)
+    for sep in (1e-5, 1e-3, 0.02, 0.11):
+        for x1 in ((0.52, 0.58, 0.53), (0.4999, 0.56, 0.53)):                              # same cell / across a cell face
+            pos = np.array([x1, np.array(x1) + sep * np.array([2.0, -1.0, 2.0]) / 3.0], dtype=np.float32)
+            got, _, _ = run(torch_cuda, NF, pos, cfg, law="newton")
+            ref, _, _ = oracle_mod.accel_variant(pos, cfg.cpd, cfg.R, cfg.eps_p, law="newton")
+            assert np.allclose(got, ref, rtol=3e-6, atol=0), (sep, x1)
+    pos = np.array([[0.3, 0.3, 0.3], [0.3, 0.3, 0.3], [0.35, 0.3, 0.3]], dtype=np.float32)     # a coincident pair: contributes 0
+    got, _, _ = run(torch_cuda, NF, pos, cfg, law="newton")
+    ref, _, _ = oracle_mod.accel_variant(pos, cfg.cpd, cfg.R, cfg.eps_p, law="newton")
+    assert np.isfinite(got).all() and np.allclose(got, ref, rtol=3e-6)
 
 
 @pytest.mark.parametrize("label,cfg", CASES, ids=[c[0] for c in CASES])

@@ -57,7 +57,6 @@ def test_null_context_calls(lib):
     assert L.nf_accel(None, None, 0, None, None) == lib.NF_EINVAL
     assert L.nf_sync(None) == lib.NF_EINVAL
     assert L.nf_set_gm(None, 1.0) == lib.NF_EINVAL
-    assert L.nf_probe_pipes(None) == lib.NF_EINVAL
     assert isinstance(L.nf_last_error(None), bytes)
 
 

@@ -17,34 +17,21 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 # ----------------------------------------------------------------------------- host logic (CPU)
-def test_slab_and_cell_index_match_the_oracle_binning(oracle_mod):
-    rng = np.random.default_rng(0)
-    pos = rng.random((5000, 3)).astype(np.float32)
-    pos[:5, 0] = [0.0, np.nextafter(np.float32(1.0), np.float32(0.0)), 1.0 / 7, 2.0 / 7, 0.999999]
-    cell, _ = oracle_mod.bin_particles(pos, 7)
-    t = torch.from_numpy(pos)
-    assert np.array_equal(slabs.cell_index(t, 7).numpy(), cell)
-    assert np.array_equal(slabs.slab_index(t, 7).numpy(), cell // 49)
+def oracle_select(oracle_mod, pos: torch.Tensor, cpd: int):
+    """a ``select(x0, nx)`` over ``pos`` from the ORACLE's binning (tests only; the product's comes
+    from nf_select_slabs)"""
+    cell, _ = oracle_mod.bin_particles(pos.numpy(), cpd)
+    xs = torch.from_numpy(cell // (cpd * cpd))
+    return (lambda x0, nx: pos[torch.remainder(xs - x0, cpd) < nx]), xs
 
 
-def test_pairs_per_slab_is_the_pair_count_identity(oracle_mod):
-    cfg = W.scaled(W.CONFIGS[3], 9)
-    pos = W.make_positions(cfg)
-    cell, _ = oracle_mod.bin_particles(pos, cfg.cpd)
-    offsets, _ = oracle_mod.cell_lists(cell, cfg.cpd)
-    counts = torch.from_numpy(np.diff(offsets))
-    per = slabs.pairs_per_slab(counts, cfg.cpd, cfg.R)
-    assert int(per.sum()) - cfg.N == oracle_mod.pair_count(offsets, cfg.cpd, cfg.R)
-    # brute force for one slab
-    n = np.diff(offsets).reshape(cfg.cpd, cfg.cpd, cfg.cpd)
-    x, tot = 4, 0
-    for j in range(cfg.cpd):
-        for k in range(cfg.cpd):
-            for a in range(-cfg.R, cfg.R + 1):
-                for b in range(-cfg.R, cfg.R + 1):
-                    for c in range(-cfg.R, cfg.R + 1):
-                        tot += n[x, j, k] * n[(x + a) % cfg.cpd, (j + b) % cfg.cpd, (k + c) % cfg.cpd]
-    assert int(per[x]) == tot
+def test_slab_runs_cover_exactly():
+    assert slabs.slab_runs([3, 4, 5], 9) == [(3, 3)]
+    assert sorted(slabs.slab_runs([8, 0, 1, 4], 9)) == [(4, 1), (8, 3)]
+    assert slabs.slab_runs([], 9) == []
+    for cpd, ss in ((5, [0, 1, 2, 3, 4]), (7, [6, 0]), (7, [1, 3, 5])):
+        got = [(x0 + i) % cpd for x0, n in slabs.slab_runs(ss, cpd) for i in range(n)]
+        assert sorted(got) == sorted(ss)
 
 
 @pytest.mark.parametrize("world", [1, 2, 3, 4, 8])
@@ -85,18 +72,20 @@ def test_halo_and_send_plans_are_consistent(cpd, R, world):
         assert all(own[x] != r for x in need)
 
 
-def test_local_with_ghosts_selects_own_and_halo():
+def test_local_with_ghosts_selects_own_and_halo(oracle_mod):
     cfg = W.scaled(W.CONFIGS[2], 9)
     pos = torch.from_numpy(W.make_positions(cfg))
     b = slabs.balance_slabs(torch.ones(9), 3)
-    xs = slabs.slab_index(pos, 9)
+    select, xs = oracle_select(oracle_mod, pos, 9)
     tot = 0
     for r in range(3):
-        own, ghost = slabs.local_with_ghosts(pos, b, 9, 2, r)
+        own, ghost = slabs.local_with_ghosts(select, b, 9, 2, r)
         x0, nx = b[r]
-        assert bool((torch.remainder(slabs.slab_index(own, 9) - x0, 9) < nx).all())
+        _, xo = oracle_select(oracle_mod, own, 9)
+        assert bool((torch.remainder(xo - x0, 9) < nx).all())
         need = set(slabs.halo_slabs(b, 9, 2, r))
-        assert set(slabs.slab_index(ghost, 9).tolist()) <= need
+        _, xg = oracle_select(oracle_mod, ghost, 9)
+        assert set(xg.tolist()) <= need
         assert ghost.shape[0] == int(sum((xs == x).sum() for x in need))
         tot += own.shape[0]
     assert tot == cfg.N
@@ -107,17 +96,24 @@ import os, sys, json
 sys.path.insert(0, os.environ["NF_ROOT"])
 import numpy as np, torch
 import torch.distributed as dist
+import oracle
 from paper_2110_11392_b200 import slabs, workloads as W
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
 cfg = W.scaled(W.CONFIGS[3], 9)
 pos = torch.from_numpy(W.make_positions(cfg))            # every rank generates the same seeded set
-counts = torch.bincount(slabs.cell_index(pos, cfg.cpd), minlength=cfg.cpd ** 3)
-bounds = slabs.balance_slabs(slabs.pairs_per_slab(counts, cfg.cpd, cfg.R), world)
-own, ghost_expect = slabs.local_with_ghosts(pos, bounds, cfg.cpd, cfg.R, rank)
-ghost = slabs.halo_exchange(own, slabs.slab_index(own, cfg.cpd), bounds, cfg.cpd, cfg.R)
+def make_select(p):                                      # the oracle's binning stands in for nf_select_slabs on the CPU
+    cell, _ = oracle.bin_particles(p.numpy(), cfg.cpd)
+    xs = torch.from_numpy(cell // (cfg.cpd * cfg.cpd))
+    return lambda x0, nx: p[torch.remainder(xs - x0, cfg.cpd) < nx]
+cell, _ = oracle.bin_particles(pos.numpy(), cfg.cpd)
+per_slab = np.bincount(cell // (cfg.cpd * cfg.cpd), minlength=cfg.cpd)
+bounds = slabs.balance_slabs(per_slab, world)
+own, ghost_expect = slabs.local_with_ghosts(make_select(pos), bounds, cfg.cpd, cfg.R, rank)
+tail = torch.full((cfg.N, 3), float("nan"))
+ghost = slabs.halo_exchange(make_select(own), own, bounds, cfg.cpd, cfg.R, recv_into=lambda n: tail[:n])
 key = lambda t: np.sort(np.ascontiguousarray(t.numpy()).view([("x", "f4"), ("y", "f4"), ("z", "f4")]).ravel(), order=["x", "y", "z"])
-ok = ghost.shape == ghost_expect.shape and np.array_equal(key(ghost), key(ghost_expect))
+ok = ghost.shape == ghost_expect.shape and np.array_equal(key(ghost), key(ghost_expect)) and ghost.data_ptr() == tail.data_ptr()
 res = torch.tensor([int(ok), own.shape[0], ghost.shape[0]])
 out = [torch.zeros_like(res) for _ in range(world)]
 dist.all_gather(out, res)
@@ -141,6 +137,45 @@ def test_halo_exchange_two_gloo_ranks(tmp_path):
     assert sum(nx for _, nx in r["bounds"]) == 9
 
 
+# ----------------------------------------------------------------------------- GPU: library-side slab support
+@pytest.mark.gpu
+def test_cell_histogram_slab_pairs_and_select_match_the_oracle(oracle_mod):
+    from paper_2110_11392_b200.binding import NearField
+    cfg = W.scaled(W.CONFIGS[3], 9)
+    pos_np = W.make_positions(cfg)
+    pos_np[:5, 0] = [0.0, np.nextafter(np.float32(1.0), np.float32(0.0)), 1.0 / 9, 2.0 / 9, 0.999999]
+    pos_np[5, 0] = 1.25                                    # outside [0, box): wrapped (reading S5)
+    pos = torch.from_numpy(pos_np).cuda()
+    cell, _ = oracle_mod.bin_particles(pos_np, cfg.cpd)
+    offsets, _ = oracle_mod.cell_lists(cell, cfg.cpd)
+    n = np.diff(offsets).reshape(cfg.cpd, cfg.cpd, cfg.cpd)
+    with NearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        counts = nf.cell_histogram(pos)
+        assert np.array_equal(counts.cpu().numpy().astype(np.int64), n.ravel())                  # A1's rule, bit exact
+        pairs, npart = nf.slab_pairs(counts)
+        pairs, npart = pairs.cpu().numpy(), npart.cpu().numpy()
+        assert np.array_equal(npart, n.sum(axis=(1, 2)))
+        assert int(pairs.sum()) - cfg.N == oracle_mod.pair_count(offsets, cfg.cpd, cfg.R)     # P7, whole box
+        x, tot = 4, 0                                                                            # brute force for one slab
+        for j in range(cfg.cpd):
+            for k in range(cfg.cpd):
+                for a in range(-cfg.R, cfg.R + 1):
+                    for b in range(-cfg.R, cfg.R + 1):
+                        for c in range(-cfg.R, cfg.R + 1):
+                            tot += n[x, j, k] * n[(x + a) % cfg.cpd, (j + b) % cfg.cpd, (k + c) % cfg.cpd]
+        assert int(pairs[x]) == tot
+        xs = cell // (cfg.cpd * cfg.cpd)
+        out = torch.empty_like(pos)
+        for x0, nx in ((0, 9), (7, 4), (3, 1), (8, 1), (2, 0)):
+            k = nf.select_slabs(pos, x0, nx, out=out)
+            want = pos_np[((xs - x0) % cfg.cpd) < nx]
+            assert k == len(want) == nf.select_slabs(pos, x0, nx)
+            assert np.array_equal(out[:k].cpu().numpy(), want)                                 # input order kept
+        assert nf.select_slabs(pos[:0], 0, 9) == 0
+        bounds = slabs.plan_slabs(nf, pos, 3)
+        assert bounds == slabs.balance_slabs(pairs, 3) and sum(nx for _, nx in bounds) == cfg.cpd
+
+
 # ----------------------------------------------------------------------------- GPU: emulated decomposition
 @pytest.mark.gpu
 @pytest.mark.parametrize("label,cfg,world", [("cfg2@13 x3", W.scaled(W.CONFIGS[2], 13), 3),
@@ -149,22 +184,30 @@ def test_halo_exchange_two_gloo_ranks(tmp_path):
                                              ("cfg2@5 (=2R+1) x2", W.scaled(W.CONFIGS[2], 5), 2)])
 def test_emulated_slab_decomposition_matches_single_call_and_oracle(oracle_mod, label, cfg, world):
     """Ranks run one after the other on one GPU (no kernel waits on another: see the profiling
-    guide): each takes its own slabs + ghosts, calls nf_accel with nf_set_sink_slabs, and the
-    union must equal the undecomposed result within the parity bar; pair counts add up exactly."""
+    guide): each takes its own slabs + ghosts (nf_select_slabs), calls nf_accel with
+    nf_set_sink_slabs, and the union must equal the undecomposed result within the parity bar;
+    pair counts add up exactly."""
     from paper_2110_11392_b200.binding import NearField
     assert torch.cuda.is_available()
     pos_np = W.make_positions(cfg)
     pos = torch.from_numpy(pos_np).cuda()
     ref, ref_pairs = oracle_mod.accel(pos_np, cfg.cpd, cfg.R, cfg.eps_p)
-    counts = torch.bincount(slabs.cell_index(pos, cfg.cpd), minlength=cfg.cpd ** 3)
-    bounds = slabs.balance_slabs(slabs.pairs_per_slab(counts, cfg.cpd, cfg.R), world)
-    xs = slabs.slab_index(pos, cfg.cpd)
+    cell, _ = oracle_mod.bin_particles(pos_np, cfg.cpd)
+    xs = torch.from_numpy(cell // (cfg.cpd * cfg.cpd)).cuda()
     got = torch.full_like(pos, float("nan"))
     pairs = 0
-    for r in range(world):
-        own, ghost = slabs.local_with_ghosts(pos, bounds, cfg.cpd, cfg.R, r)
+    with NearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as planner:
+        bounds = slabs.plan_slabs(planner, pos, world)
+
+        def select(x0, nx):
+            out = torch.empty_like(pos)
+            return out[: planner.select_slabs(pos, x0, nx, out=out)]
+
+        parts = [slabs.local_with_ghosts(select, bounds, cfg.cpd, cfg.R, r) for r in range(world)]
+    for r, (own, ghost) in enumerate(parts):
         x0, nx = bounds[r]
         idx = torch.nonzero(torch.remainder(xs - x0, cfg.cpd) < nx).ravel()
+        assert own.shape[0] == idx.numel() and torch.equal(own, pos[idx])
         allp = torch.cat([own, ghost]).contiguous()
         with NearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
             nf.set_gm(1.0 / cfg.N)                       # the global G*m, not 1/(own + ghost)
@@ -183,6 +226,28 @@ def test_emulated_slab_decomposition_matches_single_call_and_oracle(oracle_mod, 
     assert np.isfinite(g).all()
     assert d.max() <= 1e-5 * rms, f"{label}: {d.max() / rms:.3e}"
     assert np.median(d[a > 0] / a[a > 0]) <= 2e-6
+
+
+@pytest.mark.gpu
+def test_slab_nearfield_single_rank_equals_plain_call():
+    """SlabNearField with one rank (no exchange): same result as nf_accel with the same gm; the
+    own+ghost buffer is reused between steps; particles outside the rank's slabs are caught."""
+    from paper_2110_11392_b200.binding import NearField
+    cfg = W.scaled(W.CONFIGS[2], 9)
+    pos = torch.from_numpy(W.make_positions(cfg)).cuda()
+    with NearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        ref = nf.accel(pos).clone()
+        nf.sync()
+    snf = slabs.SlabNearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0, [(0, cfg.cpd)], gm=1.0 / cfg.N)
+    a1 = snf.accel(pos, validate=True).clone()
+    a2 = snf.accel(pos)
+    torch.cuda.synchronize()
+    assert torch.equal(a1, ref) and torch.equal(a2, ref) and snf.n_ghost == 0
+    snf.close()
+    half = slabs.SlabNearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0, [(0, 4)], gm=1.0 / cfg.N)
+    with pytest.raises(ValueError):
+        half.accel(pos, validate=True)
+    half.close()
 
 
 @pytest.mark.gpu
