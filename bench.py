@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- headline benchmark of the B200 near-field path (contract: task prompt, section 4).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4|all] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (A1..A6: bin, scan, scatter, schedule, interact,
 un-permute) over one synthetic particle set.  Default workload: BASELINE.json configs[3]
@@ -14,8 +14,12 @@ nf_accel_host with pinned HOST buffers (H2D + D2H inside the timed region);
 ``roofline`` = FMA-pipe issue roofline of the interaction kernel (DESIGN.md "Roofline");
 ``cpu_baseline`` = the oracle timed on the host cores on a bounded sample.
 ``--impl reference`` times the oracle (there is no other reference implementation).
-Multi-GPU: "replicas only": rank r runs the same config with seed r; no collective
-on the data path; value = total pairs / max-over-ranks time.
+``--config all`` measures configs 1, 2, 3, 5 as well and adds them under ``per_config`` (config 4
+stays the headline of the line).
+Multi-GPU (N > 1): the path shards: ONE particle set is cut into pair-balanced
+x slabs, one range per rank; a step = halo exchange of the R ghost slabs (isend/irecv over NCCL) +
+nf_accel with the own slabs as sinks; value = all pairs / max-over-ranks time ("strong").
+``--parallel replicas`` runs N independent copies instead (rank r = same config, seed r; "weak").
 """
 from __future__ import annotations
 
@@ -46,22 +50,33 @@ def _peaks():
         return {}
 
 
+def _library_state() -> str:
+    """tag of the sources the loaded library was built from (paper_2110_11392_b200/build.py)"""
+    from paper_2110_11392_b200.build import _source_hash
+    return _source_hash()[:12]
+
+
 def _ncu_traffic(config: int):
     """dram__bytes_read.sum + dram__bytes_write.sum of one k_interact launch, from the newest committed
-    ``ncu --set full`` summary of this workload under profiles/ (text; None if there is none)."""
+    ``ncu --set full`` summary of this workload under profiles/ (text; None if there is none).
+    -> (bytes, file, stale): ``stale`` unless the summary's ``# library_state:`` line names the sources
+    the library in use was built from -- a capture of another kernel state is context, not this run's traffic."""
     import glob
     import re
     best = None
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_k_interact_cfg{config}.txt"))):
-        tot, n = 0.0, 0
+        tot, n, tag = 0.0, 0, None
         with open(path) as f:
             for line in f:
+                m = re.match(r"#\s*library_state:\s*(\w+)", line)
+                if m:
+                    tag = m.group(1)
                 m = re.match(r"dram__bytes_(read|write)\.sum\s+([0-9.]+)\s+(\w+)", line)
                 if m:
                     tot += float(m.group(2)) * {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}.get(m.group(3), 1.0)
                     n += 1
         if n == 2:
-            best = (tot, os.path.relpath(path, ROOT))
+            best = (tot, os.path.relpath(path, ROOT), tag != _library_state())
     return best
 
 
@@ -142,151 +157,114 @@ def _sample_cells(cfg, n_cells: int, seed: int = 1234) -> np.ndarray:
 
 
 def time_oracle(cfg, pos, target_s: float, steps: int = 1, warmup: int = 0):
-    """oracle (as it stands) on a seeded sink-cell sample sized for ~target_s per call.
-    Returns (pairs_per_s, cores, sample description, ms_per_step)."""
+    """The oracle as it stands, timed so that the number does not depend on the sample size: its
+    binning (all particles, one thread) is timed once on its own, and the pair loop's rate is the
+    SLOPE between two seeded sink-cell samples (about 1:4), i.e. pairs added / seconds added, the
+    fixed cost of each whole call cancelling.  ``steps`` repeats of the larger sample are averaged.
+    -> dict for ``cpu_baseline`` (value = pair-loop pairs/s on all host cores) + ms per step."""
     import oracle
     cores = oracle.max_threads()
-    ppc = cfg.N / cfg.cpd ** 3
-    pairs_per_cell = ppc * ppc * (2 * cfg.R + 1) ** 3
-    guess = 1.0e8 * cores                              # pairs/s, refined by the first call
-    ncell = int(max(8, min(cfg.cpd ** 3, guess * min(target_s, 2.0) / pairs_per_cell)))
+    ncell_all = cfg.cpd ** 3
     t0 = time.perf_counter()
-    _, pairs = oracle.accel(pos, cfg.cpd, cfg.R, cfg.eps_p, sink_cells=_sample_cells(cfg, ncell))
-    dt = time.perf_counter() - t0
-    # second estimate separates the fixed (binning) cost from the pair loop
-    ncell2 = int(max(8, min(cfg.cpd ** 3, ncell * 3)))
-    t0 = time.perf_counter()
-    _, pairs2 = oracle.accel(pos, cfg.cpd, cfg.R, cfg.eps_p, sink_cells=_sample_cells(cfg, ncell2))
-    dt2 = time.perf_counter() - t0
-    rate = max((pairs2 - pairs) / max(dt2 - dt, 1e-3), 1e6) if pairs2 > pairs else pairs / dt
-    fixed = max(dt - pairs / rate, 0.0)
-    ncell3 = int(max(8, min(cfg.cpd ** 3, rate * max(target_s - fixed, 1.0) / pairs_per_cell)))
-    cells = _sample_cells(cfg, ncell3)
-    times, p3 = [], 0
-    for it in range(warmup + steps):
+    cell, _ = oracle.bin_particles(pos, cfg.cpd, cfg.box)
+    oracle.cell_lists(cell, cfg.cpd)
+    binning_s = time.perf_counter() - t0
+    counts = np.bincount(cell, minlength=ncell_all)
+    del cell
+
+    def run(cells):
         t0 = time.perf_counter()
-        _, p3 = oracle.accel(pos, cfg.cpd, cfg.R, cfg.eps_p, sink_cells=cells)
+        _, p = oracle.accel(pos, cfg.cpd, cfg.R, cfg.eps_p, sink_cells=cells)
+        return p, time.perf_counter() - t0
+
+    ppc = cfg.N / ncell_all
+    pairs_per_cell = max(ppc * ppc * (2 * cfg.R + 1) ** 3, 1.0)
+    # two samples of ~target/5 and ~4 target/5 of pair-loop time (sized from a nominal 3e8 pairs/s per core;
+    # the slope does not depend on that guess)
+    rate0 = 3.0e8 * cores
+    n1 = int(max(4, min(ncell_all, rate0 * target_s * 0.2 / pairs_per_cell)))
+    n2 = int(max(8, min(ncell_all, 4 * n1)))
+    c1, c2 = _sample_cells(cfg, n1, seed=12), _sample_cells(cfg, n2, seed=13)
+    p1, t1 = run(c1)
+    t2s, p2 = [], 0
+    for it in range(warmup + steps):
+        p2, t = run(c2)
         if it >= warmup:
-            times.append(time.perf_counter() - t0)
-    tot = sum(times)
-    sample = (f"{len(cells)} seeded random sink cells of {cfg.cpd ** 3} (all their sources), {p3:.4g} pairs per call, "
-              f"wall time of the whole oracle call incl. binning all {cfg.N} particles (~{fixed:.1f} s)")
-    return p3 * len(times) / tot, cores, sample, 1e3 * tot / len(times)
+            t2s.append(t)
+    t2 = sum(t2s) / len(t2s)
+    if p2 > p1 and t2 > t1:
+        rate = (p2 - p1) / (t2 - t1)
+        fixed = max(t1 - p1 / rate, 0.0)
+    else:                                    # the whole config fits both samples (config 1): no slope to take
+        rate, fixed = p2 / t2, 0.0
+    full_pairs = float(np.sum(counts.astype(np.float64) * _box_filter(counts.reshape(cfg.cpd, cfg.cpd, cfg.cpd), cfg.R).ravel()) - cfg.N)
+    one = _config1()
+    t0 = time.perf_counter()
+    _, p_one = oracle.accel(one[1], one[0].cpd, one[0].R, one[0].eps_p, nthreads=1)
+    single = p_one / (time.perf_counter() - t0)
+    oracle.accel(one[1], one[0].cpd, one[0].R, one[0].eps_p, nthreads=cores)            # restore the thread count
+    try:
+        affinity = len(os.sched_getaffinity(0))
+    except AttributeError:
+        affinity = os.cpu_count()
+    out = {"value": rate, "unit": UNIT, "cores": cores, "affinity_cores": affinity, "kind": "oracle",
+           "pair_loop_pairs_per_s": rate, "binning_s": binning_s, "fixed_s_per_call": fixed,
+           "extrapolated_full_config_s": binning_s + full_pairs / rate,
+           "single_thread_pairs_per_s_config1": single,
+           "sample": f"slope between two seeded sink-cell samples of {len(c1)} and {len(c2)} of {ncell_all} cells (all their sources; "
+                     f"{p1:.4g} and {p2:.4g} pairs, {t1:.2f} s and {t2:.2f} s per whole call); binning of all {cfg.N} particles timed "
+                     f"separately ({binning_s:.2f} s, one thread); extrapolated_full_config_s = binning + all {full_pairs:.4g} pairs / slope"}
+    return out, 1e3 * t2
 
 
-def bench_slabs(args, cfg, workload, dist, rank, world, local_rank, barrier):
-    """N > 1, --parallel slabs: the same particle set on every rank (seed 0), each rank owns a
-    pair-balanced range of x slabs; a step = halo exchange (NCCL isend/irecv) + nf_accel on own +
-    ghost particles with only the own slabs as sinks.  value = all pairs / max-over-ranks time."""
-    import torch
-    from paper_2110_11392_b200 import slabs
+def _config1():
     from paper_2110_11392_b200 import workloads as W
-    pos_all = torch.from_numpy(W.make_positions(cfg)).cuda()
-    counts = torch.bincount(slabs.cell_index(pos_all, cfg.cpd, cfg.box), minlength=cfg.cpd ** 3)
-    bounds = slabs.balance_slabs(slabs.pairs_per_slab(counts, cfg.cpd, cfg.R), world)
-    own, _ = slabs.local_with_ghosts(pos_all, bounds, cfg.cpd, cfg.R, rank, cfg.box)
-    own = own.contiguous()
-    del pos_all, counts
-    snf = slabs.SlabNearField(cfg.cpd, cfg.R, cfg.eps_p, cfg.box, bounds)
-    snf.nf.set_gm(1.0 / cfg.N)
-    for _ in range(args.warmup):
-        acc = snf.accel(own)
-    torch.cuda.synchronize()
-    pairs_local = snf.interaction_count()
-    sampler = ClockSampler(local_rank)
-    barrier()
-    sampler.start()
-    l0 = snf.nf.launch_count()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()
-    for _ in range(args.steps):
-        acc = snf.accel(own)
-    ev1.record()
-    barrier()
-    clocks = sampler.stop()
-    launches = snf.nf.launch_count() - l0
-    units, total_ms = aggregate_over_ranks(float(pairs_local) * args.steps, ev0.elapsed_time(ev1), dist)
-    ok = bool(torch.isfinite(acc[:: max(1, acc.shape[0] // 100003)]).all())
-    if rank == 0:
-        workload = dict(workload, parallelism=f"x-slab decomposition over {world} GPUs, R-slab halo exchange per step",
-                        slab_bounds=bounds)
-        print(json.dumps({"metric": METRIC, "value": units / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                          "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-                          "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload,
-                          "sink_updates_per_s": cfg.N * args.steps / (total_ms * 1e-3), "pairs_per_step": units / args.steps,
-                          "clocks": clocks, "e2e": None, "gpu_launches": launches, "roofline": None, "cpu_baseline": None,
-                          "ghost_particles_rank0": snf.n_ghost, "result_finite": ok}))
-    dist.destroy_process_group()
-    return 0
+    return W.CONFIGS[1], W.make_positions(W.CONFIGS[1])
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number 1..5 (default 4: CPD 135, N 157M)")
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target oracle time for cpu_baseline")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--parallel", default="replicas", choices=["replicas", "slabs"],
-                    help="N > 1: independent replicas (weak scaling, default) or ONE particle set cut into x slabs "
-                         "with an R-slab halo exchange per step (strong scaling; paper_2110_11392_b200/slabs.py)")
-    args = ap.parse_args()
-    if args.warmup < 3 and args.impl == "ours":
-        print(f"note: --warmup {args.warmup} < 3 breaks the timing rules", file=sys.stderr)
+def _box_filter(n: np.ndarray, R: int) -> np.ndarray:
+    """periodic (2R+1)^3 box filter of the occupancy histogram (accounting only: pair counts)"""
+    f = n.astype(np.float64)
+    for axis in range(3):
+        acc = np.zeros_like(f)
+        for sft in range(-R, R + 1):
+            acc += np.roll(f, sft, axis=axis)
+        f = acc
+    return f
 
-    from paper_2110_11392_b200 import workloads as W
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    base = W.CONFIGS[args.config]
-    cfg = W.Config(base.name, base.cpd, base.R, base.N, base.kind, base.eps_p, base.box, seed=rank, n_spheres=base.n_spheres)
-    workload = {"workload": f"BASELINE.json configs[{args.config - 1}]: {cfg.name} CPD={cfg.cpd} R={cfg.R} N={cfg.N} "
-                            f"eps_p={cfg.eps_p:.6g} box=1 kind={cfg.kind} seed=rank",
-                "cpd": cfg.cpd, "R": cfg.R, "N": cfg.N, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-                "l2_policy": "inputs (1.9 GB positions, ~9 GB scratch) exceed the 126 MB L2; no flush needed"
-                if cfg.N * 12 > 2 * 126e6 else "L2 flushed by writing a 256 MB buffer between timed steps"}
 
-    # ------------------------------------------------------------------ reference arm = the oracle
-    if args.impl == "reference":
-        if rank != 0:
-            return 0
-        pos = W.make_positions(cfg)
-        per_step = max(4.0, min(20.0, 150.0 / max(args.steps + args.warmup, 1)))
-        rate, cores, sample, ms = time_oracle(cfg, pos, per_step, steps=args.steps, warmup=args.warmup)
-        line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f64", "data": "synthetic", "config": workload,
-                "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
-                "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-                "gpu_launches": 0,
-                "note": "the reference arm is the CPU oracle (oracle/nf_oracle.c, double precision, OpenMP); "
-                        "each step is a bounded sink-cell sample of the workload"}
-        print(json.dumps(line))
-        return 0
+def _workload(k: int, cfg, world: int, parallel: str) -> dict:
+    par = "single GPU" if world == 1 else (f"x-slab decomposition over {world} GPUs, R-slab halo exchange per step" if parallel == "slabs"
+                                           else f"replicas x{world}")
+    return {"workload": f"BASELINE.json configs[{k - 1}]: {cfg.name} CPD={cfg.cpd} R={cfg.R} N={cfg.N} "
+                        f"eps_p={cfg.eps_p:.6g} box=1 kind={cfg.kind} seed={'0' if parallel == 'slabs' or world == 1 else 'rank'}",
+            "cpd": cfg.cpd, "R": cfg.R, "N": cfg.N, "parallelism": par,
+            "l2_policy": "inputs (1.9 GB positions, ~9 GB scratch) exceed the 126 MB L2; no flush needed"
+            if cfg.N * 12 > 2 * 126e6 else "L2 flushed by writing a 256 MB buffer between timed steps"}
 
-    # ------------------------------------------------------------------ our arm
+
+def _issued_ops_per_pair(nf, d_pos, cfg, pairs: int, rc_cells: float) -> float:
+    """FMA-pipe lane-operations the kernel ISSUES per algorithmic pair: 11 per
+    pair (3 FADD d, 3 FMA r^2, 2 FMUL rho^3, 3 FMA accumulate) in far cells and, once a close-pair
+    radius is in force, everywhere; 14 (the spline polynomial as well) only in the near cells of the
+    min-form regime.  Weighted by the near/far split of the pair count (accounting from the library's
+    cell histogram; padding and masked lanes are not counted as work on either side)."""
+    if rc_cells > 0:
+        return 11.0
+    n = nf.cell_histogram(d_pos).cpu().numpy().reshape(cfg.cpd, cfg.cpd, cfg.cpd)
+    near_cheb = min(cfg.R, max(1, int(np.ceil(2.16 * cfg.eps_p * cfg.cpd / cfg.box))))
+    near = float((n * _box_filter(n, near_cheb)).sum()) - cfg.N
+    return (14.0 * near + 11.0 * (pairs - near)) / max(pairs, 1)
+
+
+def measure(k: int, args, rank: int, world: int, local_rank: int, dist, barrier, seed: int, want_e2e: bool, cpu_seconds: float) -> dict:
+    """one config on this rank's GPU (N = 1, or one of N replicas): the JSON fields of that workload"""
     import torch
-    from paper_2110_11392_b200.build import ensure_built
-    ensure_built()                                   # no-op unless the .so is missing (fresh checkout)
-    from paper_2110_11392_b200.binding import NearField, probe_pipes
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    if args.parallel == "slabs" and world > 1:
-        return bench_slabs(args, base, workload, dist, rank, world, local_rank, barrier)
+    from paper_2110_11392_b200 import workloads as W
+    from paper_2110_11392_b200.binding import NearField
+    from paper_2110_11392_b200.pipeprobe import probe_pipes
+    base = W.CONFIGS[k]
+    cfg = W.Config(base.name, base.cpd, base.R, base.N, base.kind, base.eps_p, base.box, seed=seed, n_spheres=base.n_spheres)
     pos = W.make_positions(cfg)
     nf = NearField(cfg.cpd, cfg.R, cfg.eps_p, cfg.box)
     nf.set_option("stage_timing", 1)
@@ -305,6 +283,7 @@ def main():
             step()
         stream.synchronize()
         pairs = nf.interaction_count()
+        rc_cells = nf.close_radius()
         peaks_live = probe_pipes() if rank == 0 else None
         sampler = ClockSampler(local_rank)
         barrier()
@@ -332,7 +311,7 @@ def main():
 
     # ---- end to end through the C ABI with pinned host buffers
     e2e = None
-    if not args.no_e2e:
+    if want_e2e:
         h_pos = torch.from_numpy(pos).pin_memory()
         h_acc = torch.empty_like(h_pos).pin_memory()
         nf.accel_host_ptr(h_pos.data_ptr(), cfg.N, h_acc.data_ptr())          # warm-up (allocates staging)
@@ -345,13 +324,14 @@ def main():
         e2e_ms_local = (time.perf_counter() - t0) * 1e3
         u2, t2 = aggregate_over_ranks(float(pairs) * n_e2e, e2e_ms_local, dist)
         e2e = {"value": u2 / (t2 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": cfg.N * 12, "d2h_bytes_per_step": cfg.N * 12,
-               "steps": n_e2e, "ms_per_step": t2 / n_e2e, "api": "nf_accel_host (pinned host buffers)"}
+               "steps": n_e2e, "ms_per_step": t2 / n_e2e, "api": "nf_accel_host (pinned host buffers; H2D chunks overlap the binning)"}
         del h_pos, h_acc
-
+    out = {"value": value, "ms_per_step": total_ms / args.steps, "config": _workload(k, cfg, world, "replicas"),
+           "sink_updates_per_s": cfg.N * world * args.steps / (total_ms * 1e-3), "pairs_per_step": pairs,
+           "close_pair_radius_cells": rc_cells, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "result_finite": acc_ok}
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
-        return 0
+        nf.close()
+        return out
 
     # ---- roofline of the dominant kernel (A5): FMA-pipe issue roofline
     mp = _peaks()
@@ -359,36 +339,257 @@ def main():
     n_sm = peaks_live["sm_count"]
     peak_lane = n_sm * 128 * sm_max * 1e6                   # FP32 FMA lanes x clock
     k_ms = statistics.mean(kernel_ms)
-    traffic = _ncu_traffic(args.config)
+    traffic = _ncu_traffic(k)
     ach_lane = pairs * FMA_LANE_OPS_PER_PAIR / (k_ms * 1e-3)
-    roofline = {"bound": "alu", "kernel": "k_interact (A5 + fused A6)",
-                "achieved": ach_lane * 2 / 1e12, "peak": peak_lane * 2 / 1e12, "unit": "TFLOP/s",
-                "frac": ach_lane / peak_lane, "traffic": traffic[0] if traffic else None,
-                "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
-                "traffic_source": traffic[1] if traffic else None,
-                "convention": f"{FMA_LANE_OPS_PER_PAIR} FP32 FMA-pipe lane-ops per pair x 2 flop (SURVEY.md 8(a) note 2); "
-                              f"peak = {n_sm} SMs x 128 lanes x {sm_max:.0f} MHz x 2 (derived, DESIGN.md); "
-                              f"{FLOP_PER_PAIR} flop/pair convention -> {pairs * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12:.1f} TFLOP/s",
-                "kernel_ms": k_ms, "kernel_share_of_step": k_ms / statistics.mean(step_ms),
-                "measured_ffma_peak_lane_ops_per_s": peaks_live["ffma_lane_ops_per_s"],
-                "frac_of_measured_ffma_peak": ach_lane / peaks_live["ffma_lane_ops_per_s"],
-                "measured_ffma2_peak_lane_ops_per_s": peaks_live["ffma2_lane_ops_per_s"],
-                "measured_mufu_rsq_lane_ops_per_s": peaks_live["mufu_rsq_lane_ops_per_s"],
-                "mufu_frac": pairs / (k_ms * 1e-3) / peaks_live["mufu_rsq_lane_ops_per_s"]}
+    issued = _issued_ops_per_pair(nf, d_pos, cfg, pairs, rc_cells)
+    iss_lane = pairs * issued / (k_ms * 1e-3)
+    out["roofline"] = {
+        "bound": "alu", "kernel": "k_interact (A5 + fused A6)",
+        "achieved": ach_lane * 2 / 1e12, "peak": peak_lane * 2 / 1e12, "unit": "TFLOP/s",
+        "frac": ach_lane / peak_lane,
+        "frac_issued": iss_lane / peak_lane, "issued_fma_lane_ops_per_pair": issued,
+        "frac_issued_of_measured_ffma2_peak": iss_lane / peaks_live["ffma2_lane_ops_per_s"],
+        "traffic": traffic[0] if traffic else None,
+        "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum)",
+        "traffic_source": traffic[1] if traffic else None, "traffic_stale": traffic[2] if traffic else None,
+        "library_state": _library_state(),
+        "convention": f"frac: {FMA_LANE_OPS_PER_PAIR} FP32 FMA-pipe lane-ops per pair x 2 flop (SURVEY.md 8(a) note 2, the algorithm's count); "
+                      f"frac_issued: the {issued:.2f} lane-ops per pair the kernel issues (what ncu's sm__pipe_fma_cycles_active follows); "
+                      f"peak = {n_sm} SMs x 128 lanes x {sm_max:.0f} MHz x 2 (derived, DESIGN.md); "
+                      f"{FLOP_PER_PAIR} flop/pair convention -> {pairs * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12:.1f} TFLOP/s",
+        "kernel_ms": k_ms, "kernel_share_of_step": k_ms / statistics.mean(step_ms),
+        "measured_ffma_peak_lane_ops_per_s": peaks_live["ffma_lane_ops_per_s"],
+        "frac_of_measured_ffma_peak": ach_lane / peaks_live["ffma_lane_ops_per_s"],
+        "measured_ffma2_peak_lane_ops_per_s": peaks_live["ffma2_lane_ops_per_s"],
+        "measured_mufu_rsq_lane_ops_per_s": peaks_live["mufu_rsq_lane_ops_per_s"],
+        "measured_dfma_lane_ops_per_s": peaks_live["dfma_lane_ops_per_s"],
+        "mufu_frac": pairs / (k_ms * 1e-3) / peaks_live["mufu_rsq_lane_ops_per_s"]}
+    out["stage_ms"] = {kk: statistics.mean(st[kk] for st in stage_acc) for kk in stage_acc[0]}
+    if args.neighbours:
+        out["neighbour_steps"] = _neighbour_steps(nf, d_pos, d_acc, cfg, peaks_live)
+    nf.close()
+    del d_pos, d_acc
+    torch.cuda.empty_cache()
+    out["cpu_baseline"] = None
+    if cpu_seconds > 0:
+        out["cpu_baseline"], _ = time_oracle(cfg, pos, cpu_seconds)
+    return out
 
-    cpu = None
-    if not args.no_cpu_baseline:
-        rate, cores, sample, _ = time_oracle(cfg, pos, args.cpu_seconds)
-        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic", "config": workload,
-            "sink_updates_per_s": cfg.N * world * args.steps / (total_ms * 1e-3), "pairs_per_step": pairs,
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-            "stage_ms": {k: statistics.mean(s[k] for s in stage_acc) for k in stage_acc[0]},
-            "result_finite": acc_ok}
-    print(json.dumps(line))
+def _neighbour_steps(nf, d_pos, d_acc, cfg, peaks_live, order: int = 8) -> dict:
+    """device times of the pipeline steps either side of NearForce at this workload (Table 1:
+    TaylorForce, Kick, Drift, multipoles in Finish), each on a pinned binning (nf_bin) so that the
+    sort is timed once on its own; FP64 kernels against the measured DFMA rate."""
+    import torch
+    cml = (order + 3) * (order + 2) * (order + 1) // 6
+
+    def timed(fn, reps=3):
+        fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    res = {"order": order}
+    nf.unbin()
+    res["bin_ms"] = timed(lambda: nf.bin(d_pos))
+    M = nf.multipoles(d_pos, order)
+    res["multipoles_ms"] = timed(lambda: nf.multipoles(d_pos, order))
+    res["taylor_ms"] = timed(lambda: nf.taylor_accel(d_pos, M, order, acc=d_acc))
+    del M
+    vel = torch.zeros_like(d_pos)
+    res["kick_drift_ms"] = timed(lambda: nf.kick_drift(d_pos, vel, d_acc, 0.0, 0.0))
+    nf.unbin()
+    dfma = peaks_live["dfma_lane_ops_per_s"]
+    # algorithmic FP64 FMA-class operations per particle (DESIGN.md "Variants"): multipoles cml FMAs + (p+1)(p+2)/2
+    # products + 3p powers; Taylor ~4 per coefficient (Horner value + derivative, two folds)
+    mp_ops = cml + (order + 1) * (order + 2) // 2 + 3 * order
+    ty_ops = 4 * cml
+    res["multipoles_frac_of_dfma_peak"] = cfg.N * mp_ops / (res["multipoles_ms"] * 1e-3) / dfma
+    res["taylor_frac_of_dfma_peak"] = cfg.N * ty_ops / (res["taylor_ms"] * 1e-3) / dfma
+    res["multipoles_particles_per_s"] = cfg.N / (res["multipoles_ms"] * 1e-3)
+    res["taylor_particles_per_s"] = cfg.N / (res["taylor_ms"] * 1e-3)
+    res["kick_drift_GBps"] = cfg.N * 12 * 5 / (res["kick_drift_ms"] * 1e-3) / 1e9      # read pos, vel, acc; write pos, vel
+    res["bin_GBps_algorithmic"] = cfg.N * 72 / (res["bin_ms"] * 1e-3) / 1e9             # DESIGN.md "Kernels": 72 B per particle
+    return res
+
+
+def bench_slabs(args, k, dist, rank, world, local_rank, barrier) -> dict:
+    """ONE particle set (seed 0, every rank generates it and keeps its own slabs) over `world` GPUs: a
+    step = halo exchange of the R ghost slabs (isend/irecv: NCCL over NVLink) + nf_accel on own + ghost
+    particles with only the own slabs as sinks.  value = all pairs / max-over-ranks time (strong scaling)."""
+    import torch
+    from paper_2110_11392_b200 import slabs
+    from paper_2110_11392_b200 import workloads as W
+    from paper_2110_11392_b200.binding import NearField
+    from paper_2110_11392_b200.pipeprobe import probe_pipes
+    cfg = W.CONFIGS[k]
+    pos_np = W.make_positions(cfg)
+    with NearField(cfg.cpd, cfg.R, cfg.eps_p, cfg.box) as planner:
+        pos_all = torch.from_numpy(pos_np).cuda()
+        bounds = slabs.plan_slabs(planner, pos_all, world)           # same input on every rank: no all_reduce needed, same cuts
+        x0, nx = bounds[rank]
+        buf = torch.empty_like(pos_all)
+        n_own = planner.select_slabs(pos_all, x0, nx, out=buf)
+        own = buf[:n_own].clone()
+        del buf, pos_all
+    del pos_np
+    torch.cuda.empty_cache()
+    snf = slabs.SlabNearField(cfg.cpd, cfg.R, cfg.eps_p, cfg.box, bounds, gm=1.0 / cfg.N)
+    snf.nf.set_option("stage_timing", 1)
+    for _ in range(args.warmup):
+        acc = snf.accel(own, validate=True)
+    torch.cuda.synchronize()
+    pairs_local = snf.interaction_count()
+    rc_cells = snf.nf.close_radius()
+    peaks_live = probe_pipes() if rank == 0 else None
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    l0 = snf.nf.launch_count()
+    kernel_ms = []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        acc = snf.accel(own)
+        kernel_ms.append(snf.nf.stage_ms()["A5_interact_A6_unpermute"])
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = snf.nf.launch_count() - l0
+    units, total_ms = aggregate_over_ranks(float(pairs_local) * args.steps, ev0.elapsed_time(ev1), dist)
+    ok = bool(torch.isfinite(acc[:: max(1, acc.shape[0] // 100003)]).all())
+
+    # end to end: own particles from pinned host memory each step, accelerations back to pinned host memory
+    e2e = None
+    if not args.no_e2e:
+        h_own = own.cpu().pin_memory()
+        h_acc = torch.empty_like(h_own).pin_memory()
+        d_own = torch.empty_like(own)
+        barrier()
+        t0 = time.perf_counter()
+        n_e2e = max(1, min(args.steps, 3))
+        for _ in range(n_e2e):
+            d_own.copy_(h_own, non_blocking=True)
+            h_acc.copy_(snf.accel(d_own), non_blocking=True)
+            torch.cuda.synchronize()
+        barrier()
+        u2, t2 = aggregate_over_ranks(float(pairs_local) * n_e2e, (time.perf_counter() - t0) * 1e3, dist)
+        e2e = {"value": u2 / (t2 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": n_own * 12, "d2h_bytes_per_step": n_own * 12,
+               "steps": n_e2e, "ms_per_step": t2 / n_e2e,
+               "api": "pinned host -> device copy of the rank's particles, SlabNearField.accel (halo exchange + nf_accel), result to pinned host; bytes are rank 0's"}
+    out = {"value": units / (total_ms * 1e-3), "ms_per_step": total_ms / args.steps, "config": dict(_workload(k, cfg, world, "slabs"), slab_bounds=bounds),
+           "sink_updates_per_s": cfg.N * args.steps / (total_ms * 1e-3), "pairs_per_step": units / args.steps,
+           "close_pair_radius_cells": rc_cells, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "result_finite": ok,
+           "halo_bytes_per_step_rank0": snf.halo_bytes, "ghost_particles_rank0": snf.n_ghost, "own_particles_rank0": n_own}
+    if rank == 0:
+        mp = _peaks()
+        sm_max = float(mp.get("sm_max_mhz", 1965.0))
+        peak_lane = peaks_live["sm_count"] * 128 * sm_max * 1e6
+        k_ms = statistics.mean(kernel_ms)
+        ach = pairs_local * FMA_LANE_OPS_PER_PAIR / (k_ms * 1e-3)
+        issued = 11.0 if rc_cells > 0 else float("nan")
+        out["roofline"] = {"bound": "alu", "kernel": "k_interact (A5 + fused A6) on rank 0", "achieved": ach * 2 / 1e12, "peak": peak_lane * 2 / 1e12,
+                           "unit": "TFLOP/s", "frac": ach / peak_lane, "frac_issued": pairs_local * issued / (k_ms * 1e-3) / peak_lane,
+                           "issued_fma_lane_ops_per_pair": issued, "traffic": None, "kernel_ms": k_ms,
+                           "kernel_share_of_step": k_ms / (total_ms / args.steps), "pairs_rank0": pairs_local,
+                           "convention": f"{FMA_LANE_OPS_PER_PAIR} FP32 FMA-pipe lane-ops per pair x 2 flop; peak = SMs x 128 lanes x {sm_max:.0f} MHz x 2 of ONE GPU"}
+        out["cpu_baseline"] = None                     # timed on rank 0 at N = 1 only
+    snf.close()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="4", help="BASELINE.json config number 1..5 (default 4: CPD 135, N 157M), or 'all': "
+                                                  "config 4 as the headline plus the others under per_config")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target pair-loop time of the oracle for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--neighbours", action="store_true", help="also time nf_bin / nf_multipoles / nf_taylor_accel / nf_kick_drift at the workload")
+    ap.add_argument("--parallel", default="slabs", choices=["slabs", "replicas"],
+                    help="N > 1: ONE particle set cut into x slabs with an R-slab halo exchange per step (default; strong "
+                         "scaling; paper_2110_11392_b200/slabs.py), or independent replicas (weak scaling)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print(f"note: --warmup {args.warmup} < 3 breaks the timing rules", file=sys.stderr)
+
+    from paper_2110_11392_b200 import workloads as W
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    want_all = args.config == "all"
+    k_main = 4 if want_all else int(args.config)
+    slabs_mode = world > 1 and args.parallel == "slabs"
+
+    # ------------------------------------------------------------------ reference arm = the oracle
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        cfg = W.CONFIGS[k_main]
+        pos = W.make_positions(cfg)
+        per_step = max(4.0, min(20.0, 120.0 / max(args.steps + args.warmup, 1)))
+        cpu, ms = time_oracle(cfg, pos, per_step, steps=args.steps, warmup=args.warmup)
+        line = {"impl": "reference", "metric": METRIC, "value": cpu["value"], "unit": UNIT, "n_gpus": 0, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if slabs_mode else "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": _workload(k_main, cfg, 1, "replicas"),
+                "cpu_baseline": cpu,
+                "e2e": {"value": cpu["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0,
+                "note": "the reference arm is the CPU oracle (oracle/nf_oracle.c, double precision, OpenMP); value = its pair-loop "
+                        "rate (slope between two sink-cell samples, the same quantity as our arm's cpu_baseline.value); each step is "
+                        "one whole oracle call on the larger sample (ms_per_step)"}
+        print(json.dumps(line))
+        return 0
+
+    # ------------------------------------------------------------------ our arm
+    import torch
+    from paper_2110_11392_b200.build import ensure_built
+    ensure_built()                                   # no-op unless the libraries are missing or older than their sources
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cpu_s = 0.0 if (args.no_cpu_baseline or world > 1) else args.cpu_seconds
+    if slabs_mode:
+        res = bench_slabs(args, k_main, dist, rank, world, local_rank, barrier)
+        scaling = "strong"
+    else:
+        res = measure(k_main, args, rank, world, local_rank, dist, barrier, seed=rank, want_e2e=not args.no_e2e, cpu_seconds=cpu_s)
+        scaling = "weak"
+    per_config = None
+    if want_all and not slabs_mode:
+        per_config = {}
+        for k in (1, 2, 3, 5):
+            r = measure(k, args, rank, world, local_rank, dist, barrier, seed=rank, want_e2e=not args.no_e2e,
+                        cpu_seconds=min(cpu_s, 6.0))
+            if rank == 0:
+                per_config[str(k)] = r
+    if rank == 0:
+        line = {"metric": METRIC, "value": res.pop("value"), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": res.pop("ms_per_step"), "higher_is_better": True, "scaling": scaling, "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic"}
+        line.update(res)
+        if per_config is not None:
+            line["per_config"] = per_config
+        print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
     return 0

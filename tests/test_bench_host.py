@@ -52,8 +52,13 @@ def test_oracle_timing_leg_and_sampling():
     cells = bench._sample_cells(cfg, 50)
     assert len(cells) == 50 and len(set(cells.tolist())) == 50 and cells.max() < 9 ** 3
     assert np.array_equal(cells, bench._sample_cells(cfg, 50))
-    rate, cores, sample, ms = bench.time_oracle(cfg, pos, 0.5)
-    assert rate > 1e6 and cores >= 1 and "sink cells" in sample and ms > 0
+    cpu, ms = bench.time_oracle(cfg, pos, 0.5)
+    assert cpu["value"] > 1e6 and cpu["cores"] >= 1 and "sink-cell samples" in cpu["sample"] and ms > 0
+    assert cpu["value"] == cpu["pair_loop_pairs_per_s"] and cpu["binning_s"] > 0 and cpu["affinity_cores"] >= 1
+    assert cpu["single_thread_pairs_per_s_config1"] > 1e6 and cpu["extrapolated_full_config_s"] > 0
+    # the slope does not depend on the sample size: twice the budget gives the same rate within timing noise
+    cpu2, _ = bench.time_oracle(cfg, pos, 1.0)
+    assert 0.5 < cpu2["value"] / cpu["value"] < 2.0
 
 
 def test_reference_arm_json_contract():
@@ -64,5 +69,6 @@ def test_reference_arm_json_contract():
     assert r["impl"] == "reference" and r["unit"] == "pairs/s" and r["value"] > 0
     assert r["metric"] == "nearfield_pair_interactions_per_s" and r["higher_is_better"] is True
     assert r["cpu_baseline"]["kind"] == "oracle" and r["cpu_baseline"]["cores"] >= 1
+    assert r["cpu_baseline"]["value"] == r["value"] and "binning_s" in r["cpu_baseline"]
     assert r["e2e"]["h2d_bytes_per_step"] == 0 and r["e2e"]["value"] == r["value"]
     assert "workload" in r["config"]
