@@ -102,7 +102,19 @@ nf_status nf_accel(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_acc, voi
  */
 nf_status nf_bin(nf_ctx *ctx, const float *d_pos, int64_t N, void *cuda_stream);
 
-/* nf_unbin -- drop the pin of nf_bin (the next call sorts again). */
+/*
+ * nf_rebin -- drift-aware update of the grid order (the paper's insert list + merge, PAPER.md:356-395:
+ * "most particles stay in their cell"): d_pos holds the positions of the SAME N particles (same input
+ * order) the context last binned, moved a little (e.g. by nf_kick_drift).  Particles whose cell is
+ * unchanged keep their place among their cell's stayers (no sorting: the old order is ascending in
+ * input index); the others go through an insert list and are merged into their new cells by input
+ * index.  The result equals a full sort (nf_bin) of the new positions bit for bit -- offsets,
+ * permutation, planes -- and is pinned like nf_bin's.  How far the particles moved affects only the
+ * cost.  If the context holds no binning of N particles this is nf_bin.  Errors as nf_bin.
+ */
+nf_status nf_rebin(nf_ctx *ctx, const float *d_pos, int64_t N, void *cuda_stream);
+
+/* nf_unbin -- drop the pin of nf_bin / nf_rebin (the next call sorts again). */
 nf_status nf_unbin(nf_ctx *ctx);
 
 /*

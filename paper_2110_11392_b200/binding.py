@@ -23,7 +23,7 @@ SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", 
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
            "nf_interaction_count", "nf_debug_read", "nf_launch_count", "nf_close_radius",
            "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles", "nf_kick_drift", "nf_timestep_ratio", "nf_taylor_accel",
-           "nf_debug_delivered_pairs", "nf_bin", "nf_unbin", "nf_cell_histogram", "nf_slab_pairs", "nf_select_slabs"]
+           "nf_debug_delivered_pairs", "nf_bin", "nf_rebin", "nf_unbin", "nf_cell_histogram", "nf_slab_pairs", "nf_select_slabs"]
 
 
 class NearFieldError(RuntimeError):
@@ -91,6 +91,8 @@ def load_library() -> ctypes.CDLL:
     L.nf_debug_delivered_pairs.argtypes = [vp, vp]
     L.nf_bin.restype = i32
     L.nf_bin.argtypes = [vp, vp, i64, vp]
+    L.nf_rebin.restype = i32
+    L.nf_rebin.argtypes = [vp, vp, i64, vp]
     L.nf_unbin.restype = i32
     L.nf_unbin.argtypes = [vp]
     L.nf_cell_histogram.restype = i32
@@ -180,6 +182,15 @@ class NearField:
         st = torch.cuda.current_stream(pos.device) if stream is None else stream
         self._N = pos.shape[0]
         self._check(_L.nf_bin(self._h, pos.data_ptr(), pos.shape[0], ctypes.c_void_p(st.cuda_stream)))
+
+    def rebin(self, pos, stream=None):
+        """nf_rebin: update the kept grid order after the particles moved (insert list + merge) and pin it."""
+        import torch
+        if not (pos.is_cuda and pos.dtype == torch.float32 and pos.is_contiguous() and pos.dim() == 2 and pos.shape[1] == 3):
+            raise ValueError("pos must be a contiguous CUDA float32 tensor of shape [N,3]")
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        self._N = pos.shape[0]
+        self._check(_L.nf_rebin(self._h, pos.data_ptr(), pos.shape[0], ctypes.c_void_p(st.cuda_stream)))
 
     def unbin(self):
         self._check(_L.nf_unbin(self._h))

@@ -9,11 +9,12 @@
 static char g_static_err[256] = "";
 
 static void free_scratch(nf_ctx *c) {
-    void *ptrs[] = {c->d_key, c->d_arr, c->d_tmp_perm, c->d_perm_true, c->d_perm_pad, c->d_sorted, c->d_blk, c->d_blk_order};
+    void *ptrs[] = {c->d_key, c->d_arr, c->d_tmp_perm, c->d_perm_true, c->d_perm_pad, c->d_sorted, c->d_blk, c->d_blk_order, c->d_perm_alt, c->d_ins};
     for (void *p : ptrs) if (p) cudaFree(p);
-    c->d_key = c->d_arr = c->d_tmp_perm = c->d_perm_true = c->d_perm_pad = nullptr;
+    c->d_key = c->d_arr = c->d_tmp_perm = c->d_perm_true = c->d_perm_pad = c->d_perm_alt = c->d_ins = nullptr;
     c->d_sorted = nullptr; c->d_blk = nullptr; c->d_blk_order = nullptr;
-    c->capN = c->capPad = c->capBlk = 0;
+    c->capN = c->capPad = c->capBlk = c->capRebin = 0;
+    c->bin_valid = 0; c->bin_pinned = 0; c->have_sched = 0;
 }
 
 extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer, double box) {
@@ -89,7 +90,8 @@ extern "C" nf_status nf_destroy(nf_ctx *c) {
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
     free_scratch(c);
-    void *ptrs[] = {c->d_counts, c->d_offsets, c->d_poff, c->d_scan_blk, c->d_col_nblk, c->d_col_base, c->d_ctrl, c->d_pairs, c->d_nbr, c->d_pos_buf, c->d_acc_buf};
+    void *ptrs[] = {c->d_counts, c->d_offsets, c->d_poff, c->d_scan_blk, c->d_col_nblk, c->d_col_base, c->d_ctrl, c->d_pairs, c->d_nbr, c->d_pos_buf, c->d_acc_buf,
+                    c->d_offsets_alt, c->d_nstay};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     if (c->own_stream) cudaStreamDestroy(c->own_stream);
@@ -170,8 +172,10 @@ static nf_status bin_for(nf_ctx *c, const float *d_pos, int64_t N, cudaStream_t 
     if (rc != NF_OK) return rc;
     c->last_stream = st; c->lastN = N; c->have_last = 1;
     if (c->bin_pinned && c->bin_pos == d_pos && c->bin_N == N) return NF_OK;
-    c->bin_pinned = 0; c->have_sched = 0;
-    return nf_run_binner(c, d_pos, N, st);
+    c->bin_pinned = 0; c->have_sched = 0; c->bin_valid = 0;
+    rc = nf_run_binner(c, d_pos, N, st);
+    if (rc == NF_OK) { c->bin_valid = 1; c->bin_validN = N; }
+    return rc;
 }
 
 extern "C" nf_status nf_bin(nf_ctx *c, const float *d_pos, int64_t N, void *cuda_stream) {
@@ -185,6 +189,41 @@ extern "C" nf_status nf_bin(nf_ctx *c, const float *d_pos, int64_t N, void *cuda
     c->bin_pinned = 0;
     nf_status rc = bin_for(c, d_pos, N, (cudaStream_t)cuda_stream);
     if (rc != NF_OK) return rc;
+    c->bin_pinned = 1; c->bin_pos = d_pos; c->bin_N = N;
+    return NF_OK;
+}
+
+extern "C" nf_status nf_rebin(nf_ctx *c, const float *d_pos, int64_t N, void *cuda_stream) {
+    if (!c) return NF_EINVAL;
+    c->err[0] = 0;
+    if (N <= 0 || !d_pos || (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_rebin: bad argument (N=%lld)", (long long)N);
+        return NF_EINVAL;
+    }
+    if (!c->bin_valid || c->bin_validN != N || N > c->capN) return nf_bin(c, d_pos, N, cuda_stream);   // nothing to update: sort
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    NF_CUDA_OK(c, cudaSetDevice(c->device));
+    if (c->capRebin < N || !c->d_offsets_alt) {
+        cudaStreamSynchronize(c->last_stream);
+        if (c->d_perm_alt) cudaFree(c->d_perm_alt);
+        if (c->d_ins) cudaFree(c->d_ins);
+        c->d_perm_alt = c->d_ins = nullptr; c->capRebin = 0;
+        cudaError_t e = cudaMalloc((void **)&c->d_perm_alt, (size_t)c->capN * 4);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_ins, (size_t)c->capN * 4);
+        if (e == cudaSuccess && !c->d_offsets_alt) e = cudaMalloc((void **)&c->d_offsets_alt, (size_t)(c->ncell + 1) * 4);
+        if (e == cudaSuccess && !c->d_nstay) e = cudaMalloc((void **)&c->d_nstay, (size_t)(c->ncell + 1) * 8);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            snprintf(c->err, sizeof c->err, "nf_rebin: scratch allocation failed: %s", cudaGetErrorString(e));
+            return NF_ENOMEM;
+        }
+        c->capRebin = c->capN;
+    }
+    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    c->bin_pinned = 0; c->have_sched = 0; c->bin_valid = 0;
+    nf_status rc = nf_run_rebin(c, d_pos, N, st);
+    if (rc != NF_OK) return rc;
+    c->bin_valid = 1; c->bin_validN = N;
     c->bin_pinned = 1; c->bin_pos = d_pos; c->bin_N = N;
     return NF_OK;
 }

@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const uint32_t *__r
 // k_scan_reduce sums items in a strided arrangement, k_scan_apply in a blocked one; both cover
 // exactly the items [blockIdx*SCAN_TILE, (blockIdx+1)*SCAN_TILE), so the block totals agree.
 
-static nf_status scan_cells(nf_ctx *ctx, cudaStream_t st) {
+nf_status nf_scan_cells(nf_ctx *ctx, cudaStream_t st) {
     uint32_t n = (uint32_t)ctx->ncell;
     uint32_t nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
     k_scan_reduce<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk); ctx->launches++;
@@ -218,7 +218,7 @@ nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t
     k_key_hist<<<(n + 255) / 256, 256, 0, st>>>(d_pos, n, ctx->prm.scale, ctx->cpd, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_ctrl); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[1], st);
-    nf_status rc = scan_cells(ctx, st);
+    nf_status rc = nf_scan_cells(ctx, st);
     if (rc != NF_OK) return rc;
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[2], st);
     uint32_t *skey = (uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);

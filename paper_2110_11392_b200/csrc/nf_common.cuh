@@ -76,6 +76,12 @@ struct nf_ctx {
     int64_t capN, capPad, capBlk, capScan;
     uint32_t *d_key, *d_arr, *d_counts, *d_offsets, *d_poff, *d_tmp_perm, *d_perm_true, *d_perm_pad;
     unsigned long long *d_scan_in, *d_scan_blk;
+    // nf_rebin (allocated at its first use): the other half of the offsets / permutation double buffers,
+    // the insert list, per-cell stayer counts + bucket fill counters
+    uint32_t *d_offsets_alt, *d_perm_alt, *d_ins, *d_nstay;
+    int64_t capRebin;
+    int bin_valid;               // d_offsets / d_perm_true hold the grid order of bin_validN particles
+    int64_t bin_validN;
     float *d_sorted;             // 4 planes of capPad: x, y, z (cell units), cell key (uint32 bits)
     uint32_t *d_col_nblk, *d_col_base, *d_scan32_blk, *d_blk_order;
     NfBlockDesc *d_blk;
@@ -112,6 +118,8 @@ struct nf_ctx {
 
 // stages implemented in the other translation units
 nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st);
+nf_status nf_run_rebin(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st);
+nf_status nf_scan_cells(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st);
 nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st);
 nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st);

@@ -126,7 +126,7 @@ def test_bin_once_reuse_everywhere(torch_cuda, NF, oracle_mod):
         pinned_launches = nf.launch_count() - n1
         st = nf.stage_ms()
         assert pinned_launches <= plain_launches - 6          # key_hist, 3 scans, scatter, rank_gather not launched
-        assert st["A1_key_hist"] == 0.0 and st["A3_scatter_rank_gather"] == 0.0 and st["A5_interact_A6_unpermute"] > 0
+        assert st["A1_key_hist"] < 0.02 and st["A3_scatter_rank_gather"] < 0.02 and st["A5_interact_A6_unpermute"] > 0   # back-to-back events
         n2 = nf.launch_count()
         M_pin = nf.multipoles(d_pos, 4)
         assert nf.launch_count() - n2 == 1
@@ -161,3 +161,74 @@ def test_bin_once_reuse_everywhere(torch_cuda, NF, oracle_mod):
     assert np.linalg.norm(g - ref, axis=1).max() <= 1e-5 * rms
     with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf2:
         assert torch.equal(nf2.accel(other), b0)
+
+
+REBIN = [("cfg2 @cpd13", W.scaled(W.CONFIGS[2], 13)), ("cfg3 @cpd10", W.scaled(W.CONFIGS[3], 10)), ("cfg4 @cpd9", W.scaled(W.CONFIGS[4], 9)),
+         ("cfg5 @cpd7 R3", W.scaled(W.CONFIGS[5], 7)), ("cfg3 full", W.CONFIGS[3])]
+
+
+@pytest.mark.parametrize("label,cfg", REBIN, ids=[r[0] for r in REBIN])
+def test_rebin_equals_a_full_sort(torch_cuda, NF, oracle_mod, label, cfg):
+    """nf_rebin (insert list + merge) after the particles moved: cell offsets, the
+    permutation (ascending input index within a cell), the cell-relative planes and the padding equal
+    a full counting sort of the new positions bit for bit -- for drifts that move a few per cent of the
+    particles out of their cells, about half of them, and all of them, several steps in a row."""
+    torch = torch_cuda
+    pos, vel, _ = _state(cfg, 7)
+    vel = (vel / 0.3 * cfg.cell).astype(np.float32)               # rms 1 cell per unit time per component
+    d_pos, d_vel = torch.from_numpy(pos.copy()).cuda(), torch.from_numpy(vel).cuda()
+    zero = torch.zeros_like(d_pos)
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf, NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as fresh:
+        nf.bin(d_pos)
+        for step, dt in enumerate((0.02, 0.0, 0.4, 5.0, 0.05)):
+            before = d_pos.clone()
+            nf.kick_drift(d_pos, d_vel, zero, 0.0, dt)
+            nf.rebin(d_pos)
+            got = nf.debug_cells()
+            moved = d_pos.cpu().numpy()
+            cell, _ = oracle_mod.bin_particles(moved, cfg.cpd)
+            offsets, order = oracle_mod.cell_lists(cell, cfg.cpd)
+            assert np.array_equal(got["offsets"].astype(np.int64), offsets), (label, step)
+            assert np.array_equal(got["perm"].astype(np.int64), order), (label, step)
+            fresh.bin(d_pos)
+            ref = fresh.debug_cells()
+            for k in ("offsets", "perm", "poffsets", "sorted_key"):
+                assert np.array_equal(got[k], ref[k]), (label, step, k)
+            assert np.array_equal(got["sorted_xyz"], ref["sorted_xyz"]), (label, step)
+            if cfg.N < 2_000_000:
+                a = nf.accel(d_pos)                                 # on the updated order (pinned by nf_rebin)
+                b = fresh.accel(d_pos)
+                nf.sync(), fresh.sync()
+                assert torch.equal(a, b), (label, step)
+            old_cell, _ = oracle_mod.bin_particles(before.cpu().numpy(), cfg.cpd)
+            frac = float((old_cell != cell).mean())
+            assert (dt == 0.0) == (frac == 0.0)
+        assert frac < 0.2                                           # the last drift is a small one again
+
+
+def test_rebin_without_a_binning_and_with_another_count(torch_cuda, NF, oracle_mod):
+    torch = torch_cuda
+    cfg = W.scaled(W.CONFIGS[2], 9)
+    pos = W.make_positions(cfg)
+    d = torch.from_numpy(pos).cuda()
+    with NF(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        nf.rebin(d)                                                 # nothing held yet: a full sort
+        cell, _ = oracle_mod.bin_particles(pos, cfg.cpd)
+        offsets, order = oracle_mod.cell_lists(cell, cfg.cpd)
+        g = nf.debug_cells()
+        assert np.array_equal(g["offsets"].astype(np.int64), offsets) and np.array_equal(g["perm"].astype(np.int64), order)
+        half = d[: cfg.N // 2].contiguous()
+        nf.rebin(half)                                              # another count: a full sort again
+        c2, _ = oracle_mod.bin_particles(pos[: cfg.N // 2], cfg.cpd)
+        o2, r2 = oracle_mod.cell_lists(c2, cfg.cpd)
+        g = nf.debug_cells()
+        assert np.array_equal(g["offsets"].astype(np.int64), o2) and np.array_equal(g["perm"].astype(np.int64), r2)
+        # everything into one cell, then spread out again
+        one = ((3 + torch.rand((cfg.N // 2, 3), device="cuda")) / cfg.cpd).contiguous()
+        nf.rebin(one)
+        g = nf.debug_cells()
+        assert int(g["offsets"][-1]) == cfg.N // 2 and int(np.diff(g["offsets"].astype(np.int64)).max()) == cfg.N // 2
+        assert np.array_equal(g["perm"], np.arange(cfg.N // 2, dtype=np.uint32))
+        nf.rebin(half)
+        g = nf.debug_cells()
+        assert np.array_equal(g["offsets"].astype(np.int64), o2) and np.array_equal(g["perm"].astype(np.int64), r2)
