@@ -9,9 +9,9 @@
 static char g_static_err[256] = "";
 
 static void free_scratch(nf_ctx *c) {
-    void *ptrs[] = {c->d_key, c->d_arr, c->d_tmp_perm, c->d_perm_true, c->d_perm_pad, c->d_sorted, c->d_blk, c->d_blk_order, c->d_perm_alt, c->d_ins};
+    void *ptrs[] = {c->d_key, c->d_arr, c->d_tmp_perm, c->d_chunk_sorted, c->d_perm_true, c->d_perm_pad, c->d_sorted, c->d_blk, c->d_blk_order, c->d_perm_alt, c->d_ins};
     for (void *p : ptrs) if (p) cudaFree(p);
-    c->d_key = c->d_arr = c->d_tmp_perm = c->d_perm_true = c->d_perm_pad = c->d_perm_alt = c->d_ins = nullptr;
+    c->d_key = c->d_arr = c->d_tmp_perm = c->d_chunk_sorted = c->d_perm_true = c->d_perm_pad = c->d_perm_alt = c->d_ins = nullptr;
     c->d_sorted = nullptr; c->d_blk = nullptr; c->d_blk_order = nullptr;
     c->capN = c->capPad = c->capBlk = c->capRebin = 0;
     c->bin_valid = 0; c->bin_pinned = 0; c->have_sched = 0;
@@ -149,9 +149,10 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
     A((void **)&c->d_key, (size_t)N * 4);
     A((void **)&c->d_arr, (size_t)N * 4);
     A((void **)&c->d_tmp_perm, (size_t)capPad * 4);
+    A((void **)&c->d_chunk_sorted, (size_t)capPad * 4);
     A((void **)&c->d_perm_true, (size_t)N * 4);
     A((void **)&c->d_perm_pad, (size_t)capPad * 4);
-    A((void **)&c->d_sorted, (size_t)capPad * 16);
+    A((void **)&c->d_sorted, (size_t)capPad * 4 * NF_PLANES);
     A((void **)&c->d_blk, (size_t)capBlk * sizeof(NfBlockDesc));
     A((void **)&c->d_blk_order, (size_t)capBlk * 4);
     if (e != cudaSuccess) {

@@ -172,42 +172,81 @@ __global__ void __launch_bounds__(256) k_scatter(uint32_t N, const uint32_t *__r
     }
 }
 
-__device__ __forceinline__ float nf_axis_offset(float x, double scale) {
-    double t = (double)x * scale;
-    return (float)(t - floor(t) - 0.5);       // offset from the cell centre, cell units, [-0.5, 0.5)
+
+// Rank within the cell by ascending input index (=> stable, run-to-run deterministic order).  The
+// arrival list of a cell is cut into chunks of NF_RANK_CHUNK slots.  A slot counts the smaller indices
+// of its own chunk (<= NF_RANK_CHUNK cache-hot loads); for a cell of one chunk (every cell at the
+// paper's 30-100 per cell) that is its rank and the particle is gathered at once.  A longer cell
+// (clustered states: 10^3-10^4 per cell) would make that count O(n_c^2); instead its chunks are
+// written out SORTED and the cell goes onto a worklist, and k_rank_big adds, per slot, one binary
+// search in each of the cell's other sorted chunks: O(n_c (chunk + (n_c/chunk) log chunk)).
+#define NF_RANK_CHUNK 256
+__device__ __forceinline__ void nf_place(const float *__restrict__ pos, double scale, uint32_t cap_pad, float *__restrict__ sorted,
+                                         uint32_t *__restrict__ perm_true, uint32_t *__restrict__ perm_pad, uint32_t lo, uint32_t o0,
+                                         uint32_t rank, uint32_t me) {
+    const uint32_t dst = lo + rank;
+    nf_store_offsets(sorted, cap_pad, dst, pos + 3ull * me, scale);
+    perm_pad[dst] = me;
+    perm_true[o0 + rank] = me;
 }
 
 __global__ void __launch_bounds__(256) k_rank_gather(const float *__restrict__ pos, double scale, uint32_t cap_pad,
-                                                     const uint32_t *__restrict__ ctrl, const uint32_t *__restrict__ offsets,
+                                                     uint32_t *__restrict__ ctrl, const uint32_t *__restrict__ offsets,
                                                      const uint32_t *__restrict__ poff, const uint32_t *__restrict__ tmp_perm,
                                                      float *__restrict__ sorted, uint32_t *__restrict__ perm_true,
-                                                     uint32_t *__restrict__ perm_pad) {
+                                                     uint32_t *__restrict__ perm_pad, uint32_t *__restrict__ chunk_sorted,
+                                                     uint32_t *__restrict__ big_cells) {
     uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t npad = ctrl[3];
-    float *sx = sorted, *sy = sorted + cap_pad, *sz = sorted + 2ull * cap_pad;
     uint32_t *skey = (uint32_t *)(sorted + 3ull * cap_pad);
     if (s >= npad) {
         if (s < npad + 8 && s < cap_pad) {    // tail slack read by 16-byte aligned bulk copies
-            sx[s] = NF_BIG; sy[s] = 0.f; sz[s] = 0.f; skey[s] = NF_PAD_FLAG; perm_pad[s] = 0xffffffffu;
+            nf_store_padding(sorted, cap_pad, s); skey[s] = NF_PAD_FLAG; perm_pad[s] = 0xffffffffu;
         }
         return;
     }
     uint32_t k = skey[s];
     if (k & NF_PAD_FLAG) {
-        sx[s] = NF_BIG; sy[s] = 0.f; sz[s] = 0.f; perm_pad[s] = 0xffffffffu;
+        nf_store_padding(sorted, cap_pad, s); perm_pad[s] = 0xffffffffu;
         return;
     }
     const uint32_t lo = poff[k], o0 = offsets[k], n = offsets[k + 1] - o0;
     const uint32_t me = tmp_perm[s];
+    const uint32_t c0 = lo + ((s - lo) / NF_RANK_CHUNK) * NF_RANK_CHUNK;           // this slot's chunk: [c0, c1)
+    const uint32_t c1 = (c0 + NF_RANK_CHUNK < lo + n) ? c0 + NF_RANK_CHUNK : lo + n;
     uint32_t rank = 0;
-    for (uint32_t t = 0; t < n; ++t) rank += (tmp_perm[lo + t] < me) ? 1u : 0u;
-    const float *p = pos + 3ull * me;
-    const uint32_t dst = lo + rank;
-    sx[dst] = nf_axis_offset(p[0], scale);
-    sy[dst] = nf_axis_offset(p[1], scale);
-    sz[dst] = nf_axis_offset(p[2], scale);
-    perm_pad[dst] = me;
-    perm_true[o0 + rank] = me;
+    for (uint32_t t = c0; t < c1; ++t) rank += (tmp_perm[t] < me) ? 1u : 0u;
+    if (n <= NF_RANK_CHUNK) { nf_place(pos, scale, cap_pad, sorted, perm_true, perm_pad, lo, o0, rank, me); return; }
+    chunk_sorted[c0 + rank] = me;
+    if (s == lo) big_cells[atomicAdd(&ctrl[7], 1u)] = k;
+}
+
+// the long cells: one CTA per worklist entry strides over the cell's slots
+__global__ void __launch_bounds__(256) k_rank_big(const float *__restrict__ pos, double scale, uint32_t cap_pad,
+                                                  const uint32_t *__restrict__ ctrl, const uint32_t *__restrict__ offsets,
+                                                  const uint32_t *__restrict__ poff, const uint32_t *__restrict__ chunk_sorted,
+                                                  const uint32_t *__restrict__ big_cells, float *__restrict__ sorted,
+                                                  uint32_t *__restrict__ perm_true, uint32_t *__restrict__ perm_pad) {
+    const uint32_t nbig = ctrl[7];
+    for (uint32_t w = blockIdx.x; w < nbig; w += gridDim.x) {
+        const uint32_t k = big_cells[w];
+        const uint32_t lo = poff[k], o0 = offsets[k], n = offsets[k + 1] - o0;
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+            const uint32_t me = chunk_sorted[lo + i];
+            uint32_t rank = i % NF_RANK_CHUNK;                                     // its place in its own sorted chunk
+            for (uint32_t c0 = 0; c0 < n; c0 += NF_RANK_CHUNK) {
+                if (c0 == i - i % NF_RANK_CHUNK) continue;
+                uint32_t a = lo + c0, b = lo + ((c0 + NF_RANK_CHUNK < n) ? c0 + NF_RANK_CHUNK : n);
+                const uint32_t first = a;
+                while (a < b) {                                                    // entries of that chunk below `me`
+                    const uint32_t mid = (a + b) >> 1;
+                    if (chunk_sorted[mid] < me) a = mid + 1; else b = mid;
+                }
+                rank += a - first;
+            }
+            nf_place(pos, scale, cap_pad, sorted, perm_true, perm_pad, lo, o0, rank, me);
+        }
+    }
 }
 
 nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st) {
@@ -229,7 +268,10 @@ nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t
     if (bound > (uint64_t)ctx->capPad) bound = ctx->capPad;
     k_rank_gather<<<(uint32_t)((bound + 255) / 256), 256, 0, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl,
                                                                    ctx->d_offsets, ctx->d_poff, ctx->d_tmp_perm, ctx->d_sorted,
-                                                                   ctx->d_perm_true, ctx->d_perm_pad); ctx->launches++;
+                                                                   ctx->d_perm_true, ctx->d_perm_pad, ctx->d_chunk_sorted, ctx->d_key); ctx->launches++;
+    // (d_key is free after the scatter: it holds the worklist of long cells, at most N / NF_RANK_CHUNK entries)
+    k_rank_big<<<ctx->sm_count * 8, 256, 0, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
+                                                  ctx->d_chunk_sorted, ctx->d_key, ctx->d_sorted, ctx->d_perm_true, ctx->d_perm_pad); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[3], st);
     return NF_OK;

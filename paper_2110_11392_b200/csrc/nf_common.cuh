@@ -74,7 +74,7 @@ struct nf_ctx {
     float opt_rc;                // close-pair radius in cells; < 0 = automatic
     // scratch (grow-only)
     int64_t capN, capPad, capBlk, capScan;
-    uint32_t *d_key, *d_arr, *d_counts, *d_offsets, *d_poff, *d_tmp_perm, *d_perm_true, *d_perm_pad;
+    uint32_t *d_key, *d_arr, *d_counts, *d_offsets, *d_poff, *d_tmp_perm, *d_chunk_sorted, *d_perm_true, *d_perm_pad;
     unsigned long long *d_scan_in, *d_scan_blk;
     // nf_rebin (allocated at its first use): the other half of the offsets / permutation double buffers,
     // the insert list, per-cell stayer counts + bucket fill counters
@@ -86,6 +86,7 @@ struct nf_ctx {
     uint32_t *d_col_nblk, *d_col_base, *d_scan32_blk, *d_blk_order;
     NfBlockDesc *d_blk;
     uint32_t *d_ctrl;            // [0] work counter  [1] number of blocks  [2] bad-position flag  [3] npad
+                                 // [5] insert-list tail (nf_rebin)  [6] dense-cell count (nf_multipoles)  [7] long-cell count (rank)
                                  // [16..79] cost histogram  [96..98] float rc^2, rc, rc^-3  [100..101] u64 sum n_c^2  [104] work counter of nf_accel_f64
     unsigned long long *d_pairs;
     int32_t *d_nbr;              // debug neighbour list
@@ -161,4 +162,26 @@ __device__ __forceinline__ int nf_axis_cell(float x, double scale, int cpd, int 
     double m = fmod(I, (double)cpd);      // exact
     if (m < 0.0) m += (double)cpd;
     return (int)m;
+}
+
+// The sorted planes (d_sorted, NF_PLANES planes of capPad slots): 0-2 x, y, z offsets from the cell
+// centre in CELL units, rounded to float32 (the hot loop's operands); 3 the cell key (uint32 bits);
+// 4-6 the float32 remainders lo = (float)(offset - (double)hi), so that (double)hi + (double)lo is
+// the double-precision offset to 2^-48 -- read by the exact paths (close pairs, multipoles) in place
+// of a second gather through the permutation.
+#define NF_PLANES 7
+__device__ __forceinline__ void nf_store_offsets(float *sorted, uint32_t cap_pad, uint32_t dst, const float *p, double scale) {
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double t = (double)p[k] * scale;
+        const double off = t - floor(t) - 0.5;                 // [-0.5, 0.5), reading S5
+        const float hi = (float)off;
+        sorted[(size_t)k * cap_pad + dst] = hi;
+        sorted[(size_t)(4 + k) * cap_pad + dst] = (float)(off - (double)hi);
+    }
+}
+__device__ __forceinline__ void nf_store_padding(float *sorted, uint32_t cap_pad, uint32_t dst) {
+    sorted[dst] = NF_BIG; sorted[(size_t)cap_pad + dst] = 0.f; sorted[2ull * cap_pad + dst] = 0.f;
+#pragma unroll
+    for (int k = 4; k < 7; ++k) sorted[(size_t)k * cap_pad + dst] = 0.f;
 }

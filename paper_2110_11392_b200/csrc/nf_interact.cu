@@ -247,7 +247,7 @@ struct ProdState {       // cursor of the stage producer (block, column, z-run, 
 };
 
 struct InteractArgs {
-    const float *sx, *sy, *sz, *pos;
+    const float *sx, *sy, *sz, *lx, *ly, *lz;   // hi planes (staged into shared memory) and lo planes (close_scan only)
     const uint32_t *skey, *poff, *perm_pad, *order;
     const NfBlockDesc *blk;
     uint32_t *ctrl;
@@ -266,37 +266,32 @@ struct InteractArgs {
 
 // Close pairs (r < r_c) in double precision.  The hot loop clamps the
 // float32 r^-3 of a near cell to fmax = r_c^-3 and tracks the smallest r^2 the lane saw in that
-// cell; a lane whose minimum is below r_c^2 calls close_scan() for that one cell.  The scan
+// cell; a lane whose minimum is below r_c^2 calls close_scan() for the flagged sources.  The scan
 // repeats the loop's float32 arithmetic for d and r^2 (same operations, same order, so the same
 // decision), and for every pair with r^2 < r_c^2 returns  exact F(d) d - fmax d_float,  i.e. it
 // replaces what the hot loop added by the exact value.  The float32 cell-relative offsets of
-// the sorted planes are NOT enough for the exact value: for x < box/4 the input float32 position
+// the staged planes are NOT enough for the exact value: for x < box/4 the input float32 position
 // is finer than a float32 offset of magnitude ~0.5 cell, and 1.5e-8 cell is 3e-6 of the force
-// of a pair 0.01 cell apart.  So both particles are re-read from the caller's position array
-// through the permutation and their offsets recomputed in double; the INTEGER cell shift is
+// of a pair 0.01 cell apart.  The binner therefore keeps the float32 remainder of every offset in
+// the "lo" planes (hi + lo = the double-precision offset to 2^-48): one level of independent
+// global loads per close source, no gather through the permutation; the INTEGER cell shift is
 // added last.  Piecewise Eq. 3.  Rare (a few per cent of the sinks have such a
 // neighbour), hence noinline and out of the hot loop.
 struct CloseArgs {
-    const float *pos;          // caller's positions (input order)
-    const uint32_t *perm_pad;  // padded slot -> input index
-    double scale;              // cpd / box
-    double eps;                // eps_s in cell units
+    const float *sx, *sy, *sz;   // hi planes (global; the sink's own offsets)
+    const float *lx, *ly, *lz;   // lo planes
+    double eps;                // eps_s in cell units (0: no softening)
     double soft2;              // eps_p^2 in cell units (Plummer) or 0
     float addend;              // the loop's r^2 addend
     int law;
 };
-__device__ __forceinline__ double exact_offset(float x, double scale) {
-    const double t = (double)x * scale;
-    return t - floor(t) - 0.5;
-}
 __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, const float *ys, const float *zs, int lo, int hi,
                                         uint32_t bits, int seg /* sources per flagged segment */,
                                         float xim, float yi, float zi, float rc2, float fmax, uint32_t g_lo, uint32_t sink_slot,
                                         int a, int b, int dzc, double *corr /* shared: [3][NF_BS], this thread's column */) {
-    const uint32_t pi = K.perm_pad[sink_slot];
-    if (pi == 0xffffffffu) return;               // a padding sink (its result is never stored)
-    const float *p = K.pos + 3ull * pi;
-    const double opx = exact_offset(p[0], K.scale), opy = exact_offset(p[1], K.scale), opz = exact_offset(p[2], K.scale);
+    if (!(K.sx[sink_slot] < 0.5f * NF_BIG)) return;       // a padding sink (its result is never stored)
+    const double opx = (double)K.sx[sink_slot] + (double)K.lx[sink_slot], opy = (double)K.sy[sink_slot] + (double)K.ly[sink_slot],
+                 opz = (double)K.sz[sink_slot] + (double)K.lz[sink_slot];
     double cx = 0.0, cy = 0.0, cz = 0.0;
     while (bits) {
     const int bit = __ffs(bits) - 1;
@@ -311,12 +306,11 @@ __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, con
         if (!(r2f < rc2)) continue;
         // what the hot loop added for this pair (f clamped to fmax)
         cx -= (double)fmax * (double)dxf; cy -= (double)fmax * (double)dyf; cz -= (double)fmax * (double)dzf;
-        const uint32_t qi = K.perm_pad[g_lo + (uint32_t)s];
-        if (qi == 0xffffffffu || qi == pi) continue;      // padding never gets here (x = +BIG); self pair: F(0) = 0
-        const float *q = K.pos + 3ull * qi;
-        const double dx = (exact_offset(q[0], K.scale) - opx) + (double)a;
-        const double dy = (exact_offset(q[1], K.scale) - opy) + (double)b;
-        const double dz = (exact_offset(q[2], K.scale) - opz) + (double)dzc;
+        const uint32_t q = g_lo + (uint32_t)s;            // padding never gets here (x = +BIG)
+        if (q == sink_slot) continue;                     // the particle itself: F(0) = 0
+        const double dx = (((double)xs[s] + (double)K.lx[q]) - opx) + (double)a;
+        const double dy = (((double)ys[s] + (double)K.ly[q]) - opy) + (double)b;
+        const double dz = (((double)zs[s] + (double)K.lz[q]) - opz) + (double)dzc;
         const double r2 = dx * dx + dy * dy + dz * dz;
         if (r2 == 0.0) continue;                          // coincident particles: F(0) = 0
         const double r = sqrt(r2);
@@ -619,7 +613,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
     const float rc2 = A.dyn[3];
     const float fmax = A.dyn[2];
     CloseArgs K;
-    K.pos = A.pos; K.perm_pad = A.perm_pad; K.scale = A.prm.scale; K.eps = A.close_eps;
+    K.sx = A.sx; K.sy = A.sy; K.sz = A.sz; K.lx = A.lx; K.ly = A.ly; K.lz = A.lz; K.eps = A.close_eps;
     K.law = LAW; K.addend = A.addend; K.soft2 = (LAW == NF_SOFT_PLUMMER) ? (double)A.addend : 0.0;
     const int tid_s = (int)threadIdx.x * kS;           // this thread's first column of close_corr / tot
     float px[kS], py[kS], pz[kS];
@@ -861,8 +855,9 @@ nf_status nf_interact_setup(nf_ctx *ctx) {
 }
 
 static void fill_interact_args(nf_ctx *ctx, const float *d_pos, float *d_out, int ostride, float kfac, InteractArgs &A, int &law, int &dens) {
-    A.pos = d_pos;
+    (void)d_pos;
     A.sx = ctx->d_sorted; A.sy = ctx->d_sorted + ctx->capPad; A.sz = ctx->d_sorted + 2ull * ctx->capPad;
+    A.lx = ctx->d_sorted + 4ull * ctx->capPad; A.ly = ctx->d_sorted + 5ull * ctx->capPad; A.lz = ctx->d_sorted + 6ull * ctx->capPad;
     A.skey = (const uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
     A.poff = ctx->d_poff; A.perm_pad = ctx->d_perm_pad; A.order = ctx->d_blk_order; A.blk = ctx->d_blk;
     A.ctrl = ctx->d_ctrl; A.dyn = (const float *)(ctx->d_ctrl + 96); A.acc = d_out; A.kfac = kfac; A.prm = ctx->prm;

@@ -101,12 +101,8 @@ __global__ void __launch_bounds__(256) k_rebin_bucket(const RebinArgs A) {
 __device__ __forceinline__ void rebin_store(const RebinArgs &A, uint32_t k, uint32_t rank, uint32_t me) {
     const float *p = A.pos + 3ull * me;
     const uint32_t dst = A.poff_new[k] + rank;
-    float *sx = A.sorted, *sy = A.sorted + A.cap_pad, *sz = A.sorted + 2ull * A.cap_pad;
     uint32_t *skey = (uint32_t *)(A.sorted + 3ull * A.cap_pad);
-    const double tx = (double)p[0] * A.scale, ty = (double)p[1] * A.scale, tz = (double)p[2] * A.scale;
-    sx[dst] = (float)(tx - floor(tx) - 0.5);                    // offset from the cell centre, cell units (A3's rule)
-    sy[dst] = (float)(ty - floor(ty) - 0.5);
-    sz[dst] = (float)(tz - floor(tz) - 0.5);
+    nf_store_offsets(A.sorted, A.cap_pad, dst, p, A.scale);     // offsets from the cell centre, cell units (A3's rule)
     skey[dst] = k;
     A.perm_pad[dst] = me;
     A.perm_true[A.off_new[k] + rank] = me;
@@ -147,14 +143,13 @@ __global__ void __launch_bounds__(256) k_rebin_movers(const RebinArgs A) {
 
 __global__ void __launch_bounds__(256) k_rebin_pads(const RebinArgs A) {
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-    float *sx = A.sorted, *sy = A.sorted + A.cap_pad, *sz = A.sorted + 2ull * A.cap_pad;
     uint32_t *skey = (uint32_t *)(A.sorted + 3ull * A.cap_pad);
     if (c < (uint32_t)A.ncell) {
         const uint32_t n = A.off_new[c + 1] - A.off_new[c], p0 = A.poff_new[c], p1 = A.poff_new[c + 1];
-        for (uint32_t t = p0 + n; t < p1; ++t) { sx[t] = NF_BIG; sy[t] = 0.f; sz[t] = 0.f; skey[t] = c | NF_PAD_FLAG; A.perm_pad[t] = 0xffffffffu; }
+        for (uint32_t t = p0 + n; t < p1; ++t) { nf_store_padding(A.sorted, A.cap_pad, t); skey[t] = c | NF_PAD_FLAG; A.perm_pad[t] = 0xffffffffu; }
     } else if (c < (uint32_t)A.ncell + 8u) {                    // tail slack read by 16-byte aligned bulk copies
         const uint32_t t = A.poff_new[A.ncell] + (c - (uint32_t)A.ncell);
-        if (t < A.cap_pad) { sx[t] = NF_BIG; sy[t] = 0.f; sz[t] = 0.f; skey[t] = NF_PAD_FLAG; A.perm_pad[t] = 0xffffffffu; }
+        if (t < A.cap_pad) { nf_store_padding(A.sorted, A.cap_pad, t); skey[t] = NF_PAD_FLAG; A.perm_pad[t] = 0xffffffffu; }
     }
 }
 

@@ -137,7 +137,7 @@ def test_bin_once_reuse_everywhere(torch_cuda, NF, oracle_mod):
         dbg = nf.debug_cells()
         nf.sync()
         assert torch.equal(a_pin, a_plain) and torch.equal(M_pin, M_plain) and torch.equal(f_pin, f_plain)
-        assert np.array_equal(t_pin, t_plain)
+        assert np.allclose(t_pin, t_plain, rtol=1e-13, atol=0)      # (a double sum by atomics: order varies)
         cell, _ = oracle_mod.bin_particles(pos, cfg.cpd)
         offsets, order = oracle_mod.cell_lists(cell, cfg.cpd)
         assert np.array_equal(dbg["offsets"].astype(np.int64), offsets) and np.array_equal(dbg["perm"].astype(np.int64), order)
