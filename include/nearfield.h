@@ -256,6 +256,9 @@ nf_status nf_timestep_ratio(nf_ctx *ctx, const float *d_pos, const float *d_vel,
  * nf_accel_host -- the same through HOST buffers: copies h_pos to the device, runs
  * nf_accel, copies the result back into h_acc and synchronises (this is the end-to-end
  * call bench.py times; pinned host memory makes the copies asynchronous DMA).
+ * The host-to-device copy is cut into 8 ranges on a second stream and A1 (key +
+ * histogram) runs on each range as it lands; A2..A6 need the whole histogram and
+ * follow the last range; the device-to-host copy follows the (permuted) un-permute.
  * Errors as nf_accel, plus NF_EPOS for a non-finite position.
  */
 nf_status nf_accel_host(nf_ctx *ctx, const float *h_pos, int64_t N, float *h_acc);

@@ -78,7 +78,10 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
 #undef TRY_ALLOC
     for (int i = 0; i < 8; ++i)
         if (cudaEventCreate(&c->ev[i]) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaEventCreate failed"); return fail(NF_ECUDA); }
-    if (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaStreamCreate failed"); return fail(NF_ECUDA); }
+    if (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaStreamCreate failed"); return fail(NF_ECUDA); }
+    for (int i = 0; i < NF_HOST_CHUNKS; ++i)
+        if (cudaEventCreateWithFlags(&c->ev_chunk[i], cudaEventDisableTiming) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaEventCreate failed"); return fail(NF_ECUDA); }
     rc = nf_interact_setup(c);
     if (rc != NF_OK) return fail(rc);
     *out = c;
@@ -94,7 +97,9 @@ extern "C" nf_status nf_destroy(nf_ctx *c) {
                     c->d_offsets_alt, c->d_nstay};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (int i = 0; i < NF_HOST_CHUNKS; ++i) if (c->ev_chunk[i]) cudaEventDestroy(c->ev_chunk[i]);
     if (c->own_stream) cudaStreamDestroy(c->own_stream);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     cudaGetLastError();
     delete c;
     return NF_OK;
@@ -441,7 +446,10 @@ extern "C" nf_status nf_sync(nf_ctx *c) {
 
 extern "C" nf_status nf_accel_host(nf_ctx *c, const float *h_pos, int64_t N, float *h_acc) {
     if (!c) return NF_EINVAL;
-    if (N < 0 || (N > 0 && (!h_pos || !h_acc))) { snprintf(c->err, sizeof c->err, "nf_accel_host: bad argument"); return NF_EINVAL; }
+    if (N < 0 || (N > 0 && (!h_pos || !h_acc)) || (double)N + (double)(NF_CELL_PAD - 1) * (double)c->ncell >= 2147483640.0) {
+        snprintf(c->err, sizeof c->err, "nf_accel_host: bad argument (N=%lld)", (long long)N);
+        return NF_EINVAL;
+    }
     if (N == 0) return NF_OK;
     NF_CUDA_OK(c, cudaSetDevice(c->device));
     if (N > c->capHost) {
@@ -452,9 +460,19 @@ extern "C" nf_status nf_accel_host(nf_ctx *c, const float *h_pos, int64_t N, flo
         NF_CUDA_OK(c, cudaMalloc((void **)&c->d_acc_buf, (size_t)N * 12));
         c->capHost = N;
     }
+    // H2D in ranges with A1 behind each (nf_run_binner_host), then the rest of the path on that binning
     cudaStream_t st = c->own_stream;
-    NF_CUDA_OK(c, cudaMemcpyAsync(c->d_pos_buf, h_pos, (size_t)N * 12, cudaMemcpyHostToDevice, st));
-    nf_status rc = nf_accel(c, c->d_pos_buf, N, c->d_acc_buf, (void *)st);
+    c->err[0] = 0;
+    nf_status rc = ensure_scratch(c, N);
+    if (rc != NF_OK) return rc;
+    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    c->bin_pinned = 0; c->have_sched = 0; c->bin_valid = 0;
+    rc = nf_run_binner_host(c, h_pos, c->d_pos_buf, N, st);
+    if (rc != NF_OK) return rc;
+    c->bin_valid = 1; c->bin_validN = N;
+    c->bin_pinned = 1; c->bin_pos = c->d_pos_buf; c->bin_N = N;
+    rc = nf_accel(c, c->d_pos_buf, N, c->d_acc_buf, (void *)st);
+    c->bin_pinned = 0;                       // the staging buffer is overwritten by the next call
     if (rc != NF_OK) return rc;
     NF_CUDA_OK(c, cudaMemcpyAsync(h_acc, c->d_acc_buf, (size_t)N * 12, cudaMemcpyDeviceToHost, st));
     return nf_sync(c);

@@ -249,13 +249,9 @@ __global__ void __launch_bounds__(256) k_rank_big(const float *__restrict__ pos,
     }
 }
 
-nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st) {
+// A2 + A3 once the histogram of all N particles is complete on `st`
+static nf_status binner_finish(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st) {
     const uint32_t n = (uint32_t)N;
-    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_counts, 0, (size_t)(ctx->ncell + 1) * sizeof(uint32_t), st));
-    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_ctrl, 0, 16 * sizeof(uint32_t), st));
-    if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[0], st);
-    k_key_hist<<<(n + 255) / 256, 256, 0, st>>>(d_pos, n, ctx->prm.scale, ctx->cpd, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_ctrl); ctx->launches++;
-    NF_CUDA_OK(ctx, cudaGetLastError());
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[1], st);
     nf_status rc = nf_scan_cells(ctx, st);
     if (rc != NF_OK) return rc;
@@ -275,4 +271,37 @@ nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t
     NF_CUDA_OK(ctx, cudaGetLastError());
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[3], st);
     return NF_OK;
+}
+
+nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st) {
+    const uint32_t n = (uint32_t)N;
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_counts, 0, (size_t)(ctx->ncell + 1) * sizeof(uint32_t), st));
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_ctrl, 0, 16 * sizeof(uint32_t), st));
+    if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[0], st);
+    k_key_hist<<<(n + 255) / 256, 256, 0, st>>>(d_pos, n, ctx->prm.scale, ctx->cpd, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_ctrl); ctx->launches++;
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return binner_finish(ctx, d_pos, N, st);
+}
+
+// The binner fed from HOST memory (nf_accel_host): the positions cross PCIe in NF_HOST_CHUNKS ranges on
+// the context's copy stream and A1 runs on each range as it lands -- the histogram is additive and the
+// arrival rank only has to be unique within a cell -- so key + histogram hide behind the copy.  A2/A3
+// need the complete histogram and follow the last range.
+nf_status nf_run_binner_host(nf_ctx *ctx, const float *h_pos, float *d_pos, int64_t N, cudaStream_t st) {
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_counts, 0, (size_t)(ctx->ncell + 1) * sizeof(uint32_t), st));
+    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_ctrl, 0, 16 * sizeof(uint32_t), st));
+    if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[0], st);
+    const int64_t per = (((N + NF_HOST_CHUNKS - 1) / NF_HOST_CHUNKS) + 255) / 256 * 256;
+    for (int c = 0; c < NF_HOST_CHUNKS; ++c) {
+        const int64_t i0 = (int64_t)c * per;
+        if (i0 >= N) break;
+        const int64_t nc = (N - i0 < per) ? N - i0 : per;
+        NF_CUDA_OK(ctx, cudaMemcpyAsync(d_pos + 3 * i0, h_pos + 3 * i0, (size_t)nc * 12, cudaMemcpyHostToDevice, ctx->copy_stream));
+        NF_CUDA_OK(ctx, cudaEventRecord(ctx->ev_chunk[c], ctx->copy_stream));
+        NF_CUDA_OK(ctx, cudaStreamWaitEvent(st, ctx->ev_chunk[c], 0));
+        k_key_hist<<<(uint32_t)((nc + 255) / 256), 256, 0, st>>>(d_pos + 3 * i0, (uint32_t)nc, ctx->prm.scale, ctx->cpd, ctx->d_key + i0, ctx->d_arr + i0,
+                                                                  ctx->d_counts, ctx->d_ctrl); ctx->launches++;
+    }
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return binner_finish(ctx, d_pos, N, st);
 }

@@ -45,6 +45,8 @@
 #define NF_MIN_CTAS 4             // resident CTAs per SM the interaction kernel is compiled for
 #endif
 
+#define NF_HOST_CHUNKS 8          // nf_accel_host: ranges the H2D copy is cut into (A1 runs per range)
+
 struct NfParams {
     int cpd, R, ncell, ncol;
     double scale;        // cpd / box
@@ -94,6 +96,8 @@ struct nf_ctx {
     float *d_pos_buf, *d_acc_buf;
     int64_t capHost;
     cudaStream_t own_stream;
+    cudaStream_t copy_stream;    // nf_accel_host: H2D ranges, each followed by A1 on the compute stream
+    cudaEvent_t ev_chunk[NF_HOST_CHUNKS];
     // state of the last call
     cudaStream_t last_stream;
     int64_t lastN;
@@ -119,6 +123,7 @@ struct nf_ctx {
 
 // stages implemented in the other translation units
 nf_status nf_run_binner(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st);
+nf_status nf_run_binner_host(nf_ctx *ctx, const float *h_pos, float *d_pos, int64_t N, cudaStream_t st);
 nf_status nf_run_rebin(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st);
 nf_status nf_scan_cells(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st);

@@ -306,6 +306,13 @@ def test_host_buffer_entry_point_matches_device_one(torch_cuda, NF):
         h = nf.accel_host(pos)
         d = nf.accel(torch_cuda.from_numpy(pos).cuda()).cpu().numpy()
     assert np.array_equal(h, d)
+    # the host path copies in 8 ranges with A1 behind each: ragged ranges, fewer particles than ranges, calls in a row
+    with NF(9, 2, 0.004, 1.0) as nf:
+        for n, seed in ((5, 1), (2049, 2), (100003, 3), (7, 4)):
+            p = W.uniform(n, seed)
+            h = nf.accel_host(p)
+            d = nf.accel(torch_cuda.from_numpy(p).cuda()).cpu().numpy()
+            assert np.array_equal(h, d), n
 
 
 def test_user_stream_and_stage_times(torch_cuda, NF):
