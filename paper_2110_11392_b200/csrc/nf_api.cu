@@ -9,10 +9,11 @@
 static char g_static_err[256] = "";
 
 static void free_scratch(nf_ctx *c) {
-    void *ptrs[] = {c->d_key, c->d_arr, c->d_tmp_perm, c->d_chunk_sorted, c->d_perm_true, c->d_perm_pad, c->d_sorted, c->d_blk, c->d_blk_order, c->d_perm_alt, c->d_ins};
+    void *ptrs[] = {c->d_key, c->d_arr, c->d_tmp_perm, c->d_chunk_sorted, c->d_perm_true, c->d_perm_pad, c->d_sorted, c->d_blk, c->d_blk_order, c->d_perm_alt, c->d_ins,
+                    c->d_pair_slot};
     for (void *p : ptrs) if (p) cudaFree(p);
     c->d_key = c->d_arr = c->d_tmp_perm = c->d_chunk_sorted = c->d_perm_true = c->d_perm_pad = c->d_perm_alt = c->d_ins = nullptr;
-    c->d_sorted = nullptr; c->d_blk = nullptr; c->d_blk_order = nullptr;
+    c->d_sorted = nullptr; c->d_blk = nullptr; c->d_blk_order = nullptr; c->d_pair_slot = nullptr;
     c->capN = c->capPad = c->capBlk = c->capRebin = 0;
     c->bin_valid = 0; c->bin_pinned = 0; c->have_sched = 0;
 }
@@ -69,6 +70,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     TRY_ALLOC(c->d_counts, (size_t)(c->ncell + 1) * 4);
     TRY_ALLOC(c->d_offsets, (size_t)(c->ncell + 1) * 4);
     TRY_ALLOC(c->d_poff, (size_t)(c->ncell + 1) * 4);
+    TRY_ALLOC(c->d_poff2, (size_t)(c->ncell + 1) * 4);
     TRY_ALLOC(c->d_scan_blk, nscan * 8);
     TRY_ALLOC(c->d_col_nblk, (size_t)(c->ncol + 1) * 4);
     TRY_ALLOC(c->d_col_base, (size_t)(c->ncol + 1) * 4);
@@ -93,7 +95,7 @@ extern "C" nf_status nf_destroy(nf_ctx *c) {
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
     free_scratch(c);
-    void *ptrs[] = {c->d_counts, c->d_offsets, c->d_poff, c->d_scan_blk, c->d_col_nblk, c->d_col_base, c->d_ctrl, c->d_pairs, c->d_nbr, c->d_pos_buf, c->d_acc_buf,
+    void *ptrs[] = {c->d_counts, c->d_offsets, c->d_poff, c->d_poff2, c->d_scan_blk, c->d_col_nblk, c->d_col_base, c->d_ctrl, c->d_pairs, c->d_nbr, c->d_pos_buf, c->d_acc_buf,
                     c->d_offsets_alt, c->d_nstay};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -160,6 +162,7 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
     A((void **)&c->d_sorted, (size_t)capPad * 4 * NF_PLANES);
     A((void **)&c->d_blk, (size_t)capBlk * sizeof(NfBlockDesc));
     A((void **)&c->d_blk_order, (size_t)capBlk * 4);
+    A((void **)&c->d_pair_slot, (size_t)(capPad / 2 + 8) * 4);
     if (e != cudaSuccess) {
         cudaGetLastError();
         free_scratch(c);

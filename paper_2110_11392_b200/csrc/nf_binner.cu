@@ -73,14 +73,22 @@ __device__ __forceinline__ unsigned long long cell_item(const uint32_t *counts, 
     return ((unsigned long long)((n + (NF_CELL_PAD - 1u)) & ~(NF_CELL_PAD - 1u)) << 32) | n;
 }
 
-template <int MODE>   // 0: cells (from counts)  1: plain uint32 input widened to 64 bit
+// item c of the sink-pair scan = occupancy rounded up to an even number (from the true offsets)
+__device__ __forceinline__ unsigned long long pair_item(const uint32_t *offsets, uint32_t c) {
+    return (unsigned long long)(((offsets[c + 1] - offsets[c]) + 1u) & ~1u);
+}
+template <int MODE> __device__ __forceinline__ unsigned long long scan_item(const uint32_t *in, uint32_t c) {
+    return MODE == 0 ? cell_item(in, c) : (MODE == 1 ? (unsigned long long)in[c] : pair_item(in, c));
+}
+
+template <int MODE>   // 0: cells (from counts)  1: plain uint32 input widened to 64 bit  2: cells padded to 2 (from the true offsets)
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const uint32_t *__restrict__ in, uint32_t n,
                                                               unsigned long long *__restrict__ blk) {
     unsigned long long s = 0;
     uint32_t base = blockIdx.x * SCAN_TILE;
     for (int k = 0; k < SCAN_ITEMS; ++k) {
         uint32_t c = base + k * SCAN_THREADS + threadIdx.x;
-        if (c < n) s += (MODE == 0) ? cell_item(in, c) : (unsigned long long)in[c];
+        if (c < n) s += scan_item<MODE>(in, c);
     }
     unsigned long long tot;
     block_excl_scan(s, &tot);
@@ -111,7 +119,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const uint32_t *__r
 #pragma unroll
     for (int k = 0; k < SCAN_ITEMS; ++k) {
         uint32_t c = base + k;
-        v[k] = (c < n) ? ((MODE == 0) ? cell_item(in, c) : (unsigned long long)in[c]) : 0ull;
+        v[k] = (c < n) ? scan_item<MODE>(in, c) : 0ull;
         s += v[k];
     }
     unsigned long long ex = block_excl_scan(s, nullptr) + blk[blockIdx.x];
@@ -129,7 +137,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const uint32_t *__r
         unsigned long long tot = blk[gridDim.x];
         out_lo[n] = (uint32_t)tot;
         if (MODE == 0) { out_hi[n] = (uint32_t)(tot >> 32); ctrl[3] = (uint32_t)(tot >> 32); }
-        else ctrl[1] = (uint32_t)tot;
+        else if (MODE == 1) ctrl[1] = (uint32_t)tot;
+        else ctrl[4] = (uint32_t)tot;
     }
 }
 // k_scan_reduce sums items in a strided arrangement, k_scan_apply in a blocked one; both cover
@@ -141,6 +150,18 @@ nf_status nf_scan_cells(nf_ctx *ctx, cudaStream_t st) {
     k_scan_reduce<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk); ctx->launches++;
     k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(ctx->d_scan_blk, nblk); ctx->launches++;
     k_scan_apply<0><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_counts, n, ctx->d_scan_blk, ctx->d_offsets, ctx->d_poff, ctx->d_ctrl); ctx->launches++;
+    NF_CUDA_OK(ctx, cudaGetLastError());
+    return NF_OK;
+}
+
+// exclusive scan of the cell occupancies rounded up to even -> d_poff2 (the sink order: two sinks per
+// thread, never straddling a cell); the total also goes to ctrl[4]
+nf_status nf_scan_pairs(nf_ctx *ctx, cudaStream_t st) {
+    uint32_t n = (uint32_t)ctx->ncell;
+    uint32_t nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
+    k_scan_reduce<2><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_offsets, n, ctx->d_scan_blk); ctx->launches++;
+    k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(ctx->d_scan_blk, nblk); ctx->launches++;
+    k_scan_apply<2><<<nblk, SCAN_THREADS, 0, st>>>(ctx->d_offsets, n, ctx->d_scan_blk, ctx->d_poff2, nullptr, ctx->d_ctrl); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;
 }

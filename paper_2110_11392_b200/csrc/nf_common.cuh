@@ -58,8 +58,8 @@ struct NfParams {
 
 struct NfBlockDesc {     // one sink work item: <= NF_BS consecutive padded slots of one z-column
     uint32_t col;        // cx*cpd + cy
-    uint32_t s0;         // first padded slot
-    uint32_t cnt;        // number of slots
+    uint32_t s0;         // first slot in the SINK order (cells padded to 2 slots; d_pair_slot maps a pair to its padded slot)
+    uint32_t cnt;        // number of sink-order slots
     uint32_t cost;       // estimated cost (sinks x sources in the z-window of the home column), saturating
 };
 
@@ -86,8 +86,11 @@ struct nf_ctx {
     int64_t bin_validN;
     float *d_sorted;             // 4 planes of capPad: x, y, z (cell units), cell key (uint32 bits)
     uint32_t *d_col_nblk, *d_col_base, *d_scan32_blk, *d_blk_order;
+    uint32_t *d_poff2;           // sink order: exclusive scan of the occupancies rounded up to even (A4)
+    uint32_t *d_pair_slot;       // sink pair i (sink-order slots 2i, 2i+1) -> padded slot of its first sink (A4)
     NfBlockDesc *d_blk;
     uint32_t *d_ctrl;            // [0] work counter  [1] number of blocks  [2] bad-position flag  [3] npad
+                                 // [4] sink-order slot count
                                  // [5] insert-list tail (nf_rebin)  [6] dense-cell count (nf_multipoles)  [7] long-cell count (rank)
                                  // [16..79] cost histogram  [96..98] float rc^2, rc, rc^-3  [100..101] u64 sum n_c^2  [104] work counter of nf_accel_f64
     unsigned long long *d_pairs;
@@ -141,6 +144,7 @@ nf_status nf_run_cell_histogram(nf_ctx *ctx, const float *d_pos, int64_t N, int3
 nf_status nf_run_slab_pairs(nf_ctx *ctx, const int32_t *d_counts, long long *d_pairs, long long *d_npart, cudaStream_t st);
 nf_status nf_run_select_slabs(nf_ctx *ctx, const float *d_pos, int64_t N, int x0, int nx, float *d_out, uint32_t *d_blk, cudaStream_t st);
 nf_status nf_interact_setup(nf_ctx *ctx);
+nf_status nf_scan_pairs(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st);
 
 // ---- device helpers shared by the kernels -------------------------------------------------

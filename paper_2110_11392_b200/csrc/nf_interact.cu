@@ -66,8 +66,12 @@ __device__ __forceinline__ float mufu_rsq(float x) {
 }
 
 // ------------------------------------------------------------------------------ A4: scheduler
-// Sink work items: every z-column (cx,cy) is cut into blocks of consecutive PADDED grid-order
-// slots, balanced within the column ("sink particles are arranged into blocks").
+// Sink work items: every z-column (cx,cy) is cut into blocks of consecutive grid-order sinks,
+// balanced within the column ("sink particles are arranged into blocks").  Sinks are
+// counted in the SINK ORDER: cells padded to 2 slots, not to the 4 of the source planes -- a thread
+// holds the two sinks of one pair, which must share a cell, but a sink lane spent on padding is
+// wasted, and at 40 per cell padding to 4 wastes 9 % of them against 1 % for 2.  k_pair_slots maps
+// sink pair i to the padded slot of its first sink.
 // sink slabs: only columns whose x cell index lies in the periodic range [x0, x0 + nx) hold sinks
 // (slab decomposition); the other columns are sources only (ghost slabs).
 __device__ __forceinline__ bool nf_sink_slab(int cx, int cpd, int x0, int nx) {
@@ -75,6 +79,16 @@ __device__ __forceinline__ bool nf_sink_slab(int cx, int cpd, int x0, int nx) {
     if (d < 0) d += cpd;
     return d < nx;
 }
+__global__ void __launch_bounds__(256) k_pair_slots(uint32_t cap_pad, const uint32_t *__restrict__ ctrl, const uint32_t *__restrict__ skey,
+                                                    const uint32_t *__restrict__ offsets, const uint32_t *__restrict__ poff,
+                                                    const uint32_t *__restrict__ poff2, uint32_t *__restrict__ pair_slot) {
+    const uint32_t s = 2u * (blockIdx.x * blockDim.x + threadIdx.x);      // even padded slots: cells start on multiples of 4
+    if (s >= ctrl[3]) return;
+    const uint32_t k = skey[s] & ~NF_PAD_FLAG;
+    const uint32_t t = s - poff[k];
+    if (t < offsets[k + 1] - offsets[k]) pair_slot[(poff2[k] + t) >> 1] = s;
+}
+
 __global__ void __launch_bounds__(256) k_col_blocks(int ncol, int cpd, int x0, int nx, const uint32_t *__restrict__ poff, uint32_t *__restrict__ col_nblk) {
     int col = blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= ncol) return;
@@ -198,10 +212,18 @@ nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st) {
         k_choose_rc<<<1, 32, 0, st>>>(sum2, (double)N, plummer ? ep : ctx->prm.eps_cells, plummer ? ep * ep : 0.0, ctx->law, ctx->opt_rc,
                                       (float *)(ctx->d_ctrl + 96)); ctx->launches++;
     }
-    k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->slab_x0, ctx->slab_nx, ctx->d_poff, ctx->d_col_nblk); ctx->launches++;
-    nf_status rc = nf_scan_u32(ctx, ctx->d_col_nblk, (uint32_t)ncol, ctx->d_col_base, st);
+    nf_status rc = nf_scan_pairs(ctx, st);
     if (rc != NF_OK) return rc;
-    k_fill_blocks<<<(ncol + 127) / 128, 128, 0, st>>>(ncol, ctx->cpd, ctx->d_poff, ctx->d_col_nblk, ctx->d_col_base, ctx->d_blk, ctx->R); ctx->launches++;
+    {
+        uint64_t bound = (uint64_t)N + (uint64_t)(NF_CELL_PAD - 1) * (uint64_t)ctx->ncell + 8;      // of the padded slot count, as in the binner
+        if (bound > (uint64_t)ctx->capPad) bound = ctx->capPad;
+        k_pair_slots<<<(uint32_t)((bound / 2 + 255) / 256), 256, 0, st>>>((uint32_t)ctx->capPad, ctx->d_ctrl, (const uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad),
+                                                                          ctx->d_offsets, ctx->d_poff, ctx->d_poff2, ctx->d_pair_slot); ctx->launches++;
+    }
+    k_col_blocks<<<(ncol + 255) / 256, 256, 0, st>>>(ncol, ctx->cpd, ctx->slab_x0, ctx->slab_nx, ctx->d_poff2, ctx->d_col_nblk); ctx->launches++;
+    rc = nf_scan_u32(ctx, ctx->d_col_nblk, (uint32_t)ncol, ctx->d_col_base, st);
+    if (rc != NF_OK) return rc;
+    k_fill_blocks<<<(ncol + 127) / 128, 128, 0, st>>>(ncol, ctx->cpd, ctx->d_poff2, ctx->d_col_nblk, ctx->d_col_base, ctx->d_blk, ctx->R); ctx->launches++;
     const uint32_t bound = (uint32_t)ctx->capBlk;
     if (ctx->opt_heavy_first) {
         uint32_t *hist = ctx->d_ctrl + 16;   // 64 words
@@ -249,6 +271,7 @@ struct ProdState {       // cursor of the stage producer (block, column, z-run, 
 struct InteractArgs {
     const float *sx, *sy, *sz, *lx, *ly, *lz;   // hi planes (staged into shared memory) and lo planes (close_scan only)
     const uint32_t *skey, *poff, *perm_pad, *order;
+    const uint32_t *pair_slot;                  // sink pair -> padded slot of its first sink
     const NfBlockDesc *blk;
     uint32_t *ctrl;
     const float *dyn;        // [0] rc^2 (cell units^2; 0 = no close-pair radius, use the min form)  [1] rc  [2] rc^-3
@@ -344,6 +367,7 @@ __device__ __forceinline__ float fmin3(float a, float b, float c) {
 // multiple of 4; cells start on 16-byte boundaries) against the NF_SINKS sinks of this thread:
 // four sources per LDS.128 and plane, shared by the thread's sinks.
 constexpr int kS = NF_SINKS;
+static_assert(NF_SINKS == 2, "the sink order is made of pairs: two sinks per thread");
 constexpr int kQuads = NF_QUADS_PER_TRIP;
 constexpr int kShortPass = 96;                       // passes up to this many sources flag close pairs per pass, longer ones per trip
 template <int MODE, bool TRIPBITS, int LAW, bool DENS>
@@ -563,8 +587,8 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                 q.col = d.col; q.s0 = d.s0; q.cnt = d.cnt;
                 q.ci = (int)(d.col / (uint32_t)cpd); q.cj = (int)(d.col % (uint32_t)cpd);
                 const int colbase = (int)d.col * cpd;
-                q.Z1 = (int)(A.skey[d.s0] & ~NF_PAD_FLAG) - colbase;
-                q.U1 = (int)(A.skey[d.s0 + d.cnt - 1] & ~NF_PAD_FLAG) - colbase + R;
+                q.Z1 = (int)(A.skey[A.pair_slot[d.s0 >> 1]] & ~NF_PAD_FLAG) - colbase;
+                q.U1 = (int)(A.skey[A.pair_slot[(d.s0 + d.cnt - 1) >> 1]] & ~NF_PAD_FLAG) - colbase + R;
                 q.a = -R; q.b = -R; q.u = q.Z1 - R; q.flags = NF_F_NEWBLOCK; q.mode = 1;
             }
             if (q.mode == 1) issue_run(q);           // (only right after a block start or an empty run: not prefetched)
@@ -606,8 +630,8 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
     };
 
     // =============================== consumer warps ==========================================
-    // Thread t of warp w holds the kS sinks at slots s0 + (32 w + t) kS + j of the block (adjacent
-    // slots: cells are padded to 4 slots and blocks start on multiples of 4, so they share a cell).
+    // Thread t of warp w holds the kS sinks of pair (s0 + (32 w + t) kS) / 2 of the sink order: two
+    // adjacent padded slots of one cell (the second may be the padding slot of an odd cell).
     const float2 c0 = make_float2(A.prm.c0, A.prm.c0), c1 = make_float2(A.prm.c1, A.prm.c1), c2 = make_float2(A.prm.c2, A.prm.c2);
     const int near_cheb = A.near_cheb, kahan = A.prm.kahan;
     const float rc2 = A.dyn[3];
@@ -664,7 +688,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
         if (flags & NF_F_NEWBLOCK) {
             const uint32_t off = (uint32_t)(warp * 32 + lane) * kS;
             valid = off < S.hdr.cnt;
-            slot = S.hdr.s0 + (valid ? off : 0u);
+            slot = A.pair_slot[(S.hdr.s0 + (valid ? off : 0u)) >> 1];
             const int colbase = (int)S.hdr.col * cpd;
             zl = (int)(A.skey[slot] & ~NF_PAD_FLAG) - colbase;
 #pragma unroll
@@ -859,7 +883,7 @@ static void fill_interact_args(nf_ctx *ctx, const float *d_pos, float *d_out, in
     A.sx = ctx->d_sorted; A.sy = ctx->d_sorted + ctx->capPad; A.sz = ctx->d_sorted + 2ull * ctx->capPad;
     A.lx = ctx->d_sorted + 4ull * ctx->capPad; A.ly = ctx->d_sorted + 5ull * ctx->capPad; A.lz = ctx->d_sorted + 6ull * ctx->capPad;
     A.skey = (const uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
-    A.poff = ctx->d_poff; A.perm_pad = ctx->d_perm_pad; A.order = ctx->d_blk_order; A.blk = ctx->d_blk;
+    A.poff = ctx->d_poff; A.perm_pad = ctx->d_perm_pad; A.order = ctx->d_blk_order; A.blk = ctx->d_blk; A.pair_slot = ctx->d_pair_slot;
     A.ctrl = ctx->d_ctrl; A.dyn = (const float *)(ctx->d_ctrl + 96); A.acc = d_out; A.kfac = kfac; A.prm = ctx->prm;
     A.prm.kahan = ctx->opt_kahan;
     A.ostride = ostride;
