@@ -71,6 +71,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     TRY_ALLOC(c->d_offsets, (size_t)(c->ncell + 1) * 4);
     TRY_ALLOC(c->d_poff, (size_t)(c->ncell + 1) * 4);
     TRY_ALLOC(c->d_poff2, (size_t)(c->ncell + 1) * 4);
+    TRY_ALLOC(c->d_mp_hist, 2064 * 4);      // occupancy classes of nf_multipoles (NFM_NCLASS + 1 <= 2064)
     TRY_ALLOC(c->d_scan_blk, nscan * 8);
     TRY_ALLOC(c->d_col_nblk, (size_t)(c->ncol + 1) * 4);
     TRY_ALLOC(c->d_col_base, (size_t)(c->ncol + 1) * 4);
@@ -95,7 +96,7 @@ extern "C" nf_status nf_destroy(nf_ctx *c) {
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
     free_scratch(c);
-    void *ptrs[] = {c->d_counts, c->d_offsets, c->d_poff, c->d_poff2, c->d_scan_blk, c->d_col_nblk, c->d_col_base, c->d_ctrl, c->d_pairs, c->d_nbr, c->d_pos_buf, c->d_acc_buf,
+    void *ptrs[] = {c->d_counts, c->d_offsets, c->d_poff, c->d_poff2, c->d_mp_hist, c->d_scan_blk, c->d_col_nblk, c->d_col_base, c->d_ctrl, c->d_pairs, c->d_nbr, c->d_pos_buf, c->d_acc_buf,
                     c->d_offsets_alt, c->d_nstay};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);

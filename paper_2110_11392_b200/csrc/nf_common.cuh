@@ -86,6 +86,7 @@ struct nf_ctx {
     int64_t bin_validN;
     float *d_sorted;             // 4 planes of capPad: x, y, z (cell units), cell key (uint32 bits)
     uint32_t *d_col_nblk, *d_col_base, *d_scan32_blk, *d_blk_order;
+    uint32_t *d_mp_hist;         // nf_multipoles: occupancy-class histogram of the cells (260 words)
     uint32_t *d_poff2;           // sink order: exclusive scan of the occupancies rounded up to even (A4)
     uint32_t *d_pair_slot;       // sink pair i (sink-order slots 2i, 2i+1) -> padded slot of its first sink (A4)
     NfBlockDesc *d_blk;

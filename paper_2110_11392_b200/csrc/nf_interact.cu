@@ -308,47 +308,67 @@ struct CloseArgs {
     float addend;              // the loop's r^2 addend
     int law;
 };
+// double-precision r^-1 from the float32 seed by two Newton steps (relative error ~1e-14; no DP sqrt, no DP division)
+__device__ __forceinline__ double rsqrt_f64(double x) {
+    double y = (double)mufu_rsq((float)x);
+    const double hx = 0.5 * x;
+    y = y * fma(-hx * y, y, 1.5);
+    y = y * fma(-hx * y, y, 1.5);
+    return y;
+}
 __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, const float *ys, const float *zs, int lo, int hi,
-                                        uint32_t bits, int seg /* sources per flagged segment */,
+                                        uint32_t bits, int seg /* sources per flagged segment: a multiple of 4 */,
+                                        float pxh, float pyh, float pzh /* the sink's own float32 offsets */,
                                         float xim, float yi, float zi, float rc2, float fmax, uint32_t g_lo, uint32_t sink_slot,
                                         int a, int b, int dzc, double *corr /* shared: [3][NF_BS], this thread's column */) {
-    if (!(K.sx[sink_slot] < 0.5f * NF_BIG)) return;       // a padding sink (its result is never stored)
-    const double opx = (double)K.sx[sink_slot] + (double)K.lx[sink_slot], opy = (double)K.sy[sink_slot] + (double)K.ly[sink_slot],
-                 opz = (double)K.sz[sink_slot] + (double)K.lz[sink_slot];
+    if (!(pxh < 0.5f * NF_BIG)) return;                   // a padding sink (its result is never stored)
+    const double opx = (double)pxh + (double)K.lx[sink_slot], opy = (double)pyh + (double)K.ly[sink_slot], opz = (double)pzh + (double)K.lz[sink_slot];
+    const double ie = K.eps > 0.0 ? 1.0 / K.eps : 0.0, ie3 = ie * ie * ie;
+    const float2 nx = make_float2(-xim, -xim), ny = make_float2(-yi, -yi), nz = make_float2(-zi, -zi), tau = make_float2(K.addend, K.addend);
     double cx = 0.0, cy = 0.0, cz = 0.0;
     while (bits) {
-    const int bit = __ffs(bits) - 1;
-    bits &= bits - 1u;
-    const int s0 = lo + bit * seg;
-    const int s1 = (s0 + seg < hi) ? s0 + seg : hi;
-    for (int s = s0; s < s1; ++s) {
-        const float dxf = __fadd_rn(xs[s], -xim), dyf = __fadd_rn(ys[s], -yi), dzf = __fadd_rn(zs[s], -zi);
-        float r2f = __fmaf_rn(dxf, dxf, K.addend);
-        r2f = __fmaf_rn(dyf, dyf, r2f);
-        r2f = __fmaf_rn(dzf, dzf, r2f);
-        if (!(r2f < rc2)) continue;
-        // what the hot loop added for this pair (f clamped to fmax)
-        cx -= (double)fmax * (double)dxf; cy -= (double)fmax * (double)dyf; cz -= (double)fmax * (double)dzf;
-        const uint32_t q = g_lo + (uint32_t)s;            // padding never gets here (x = +BIG)
-        if (q == sink_slot) continue;                     // the particle itself: F(0) = 0
-        const double dx = (((double)xs[s] + (double)K.lx[q]) - opx) + (double)a;
-        const double dy = (((double)ys[s] + (double)K.ly[q]) - opy) + (double)b;
-        const double dz = (((double)zs[s] + (double)K.lz[q]) - opz) + (double)dzc;
-        const double r2 = dx * dx + dy * dy + dz * dz;
-        if (r2 == 0.0) continue;                          // coincident particles: F(0) = 0
-        const double r = sqrt(r2);
-        double f;
-        if (K.law == NF_SOFT_PLUMMER) {
-            const double s2 = r2 + K.soft2;               // Eq. 2
-            f = 1.0 / (s2 * sqrt(s2));
-        } else if (r < K.eps) {
-            const double u = r / K.eps;
-            f = (10.0 - 15.0 * u + 6.0 * u * u) / (K.eps * K.eps * K.eps);
-        } else {
-            f = 1.0 / (r2 * r);
+        const int bit = __ffs(bits) - 1;
+        bits &= bits - 1u;
+        const int s0 = lo + bit * seg;
+        const int s1 = (s0 + seg < hi) ? s0 + seg : hi;
+        for (int sq = s0; sq < s1; sq += 4) {             // four sources at a time, the hot loop's packed arithmetic (same bits, same decision)
+            const float4 X = *reinterpret_cast<const float4 *>(xs + sq), Y = *reinterpret_cast<const float4 *>(ys + sq),
+                         Z = *reinterpret_cast<const float4 *>(zs + sq);
+            const float2 dxa = __fadd2_rn(make_float2(X.x, X.y), nx), dxb = __fadd2_rn(make_float2(X.z, X.w), nx);
+            const float2 dya = __fadd2_rn(make_float2(Y.x, Y.y), ny), dyb = __fadd2_rn(make_float2(Y.z, Y.w), ny);
+            const float2 dza = __fadd2_rn(make_float2(Z.x, Z.y), nz), dzb = __fadd2_rn(make_float2(Z.z, Z.w), nz);
+            float2 ra = __ffma2_rn(dxa, dxa, tau), rb = __ffma2_rn(dxb, dxb, tau);
+            ra = __ffma2_rn(dya, dya, ra); rb = __ffma2_rn(dyb, dyb, rb);
+            ra = __ffma2_rn(dza, dza, ra); rb = __ffma2_rn(dzb, dzb, rb);
+            uint32_t m4 = (ra.x < rc2 ? 1u : 0u) | (ra.y < rc2 ? 2u : 0u) | (rb.x < rc2 ? 4u : 0u) | (rb.y < rc2 ? 8u : 0u);
+            while (m4) {
+                const int k = __ffs(m4) - 1;
+                m4 &= m4 - 1u;
+                const int s = sq + k;
+                const float dxf = k == 0 ? dxa.x : (k == 1 ? dxa.y : (k == 2 ? dxb.x : dxb.y));
+                const float dyf = k == 0 ? dya.x : (k == 1 ? dya.y : (k == 2 ? dyb.x : dyb.y));
+                const float dzf = k == 0 ? dza.x : (k == 1 ? dza.y : (k == 2 ? dzb.x : dzb.y));
+                // what the hot loop added for this pair (f clamped to fmax)
+                cx -= (double)fmax * (double)dxf; cy -= (double)fmax * (double)dyf; cz -= (double)fmax * (double)dzf;
+                const uint32_t q = g_lo + (uint32_t)s;        // padding never gets here (x = +BIG)
+                if (q == sink_slot) continue;                 // the particle itself: F(0) = 0
+                const double dx = (((double)xs[s] + (double)K.lx[q]) - opx) + (double)a;
+                const double dy = (((double)ys[s] + (double)K.ly[q]) - opy) + (double)b;
+                const double dz = (((double)zs[s] + (double)K.lz[q]) - opz) + (double)dzc;
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                if (r2 == 0.0) continue;                      // coincident particles: F(0) = 0
+                double f;
+                if (K.law == NF_SOFT_PLUMMER) {
+                    const double y = rsqrt_f64(r2 + K.soft2);     // Eq. 2
+                    f = y * y * y;
+                } else {
+                    const double y = rsqrt_f64(r2);
+                    const double u = r2 * y * ie;                 // r / eps_s (0 without softening)
+                    f = (u < 1.0 && K.eps > 0.0) ? (10.0 + u * (-15.0 + 6.0 * u)) * ie3 : y * y * y;      // Eq. 3
+                }
+                cx += f * dx; cy += f * dy; cz += f * dz;
+            }
         }
-        cx += f * dx; cy += f * dy; cz += f * dz;
-    }
     }
     corr[0] += cx; corr[NF_BS] += cy; corr[2 * NF_BS] += cz;
 }
@@ -779,8 +799,8 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
 #pragma unroll
                     for (int j = 0; j < kS; ++j)
                         if (bits[j])
-                            close_scan(K, S.xs, S.ys, S.zs, lo, lo + n, bits[j], seg, xim[j], yi[j], zi[j], rc2, fmax, S.hdr.g_lo, slot + j, ha, hb, dzc,
-                                       &close_corr[0][tid_s + j]);
+                            close_scan(K, S.xs, S.ys, S.zs, lo, lo + n, bits[j], seg, px[j], py[j], pz[j], xim[j], yi[j], zi[j], rc2, fmax, S.hdr.g_lo, slot + j,
+                                       ha, hb, dzc, &close_corr[0][tid_s + j]);
                 }
             };
             // cells cz0 + i with (i div W) even are "A" cells; each takes the cell W further on as partner

@@ -35,7 +35,8 @@ struct MultipoleArgs {
     double *M;
     double scale, cellsz;
     int ncell, order, cml;
-    uint32_t *dense, *ndense;         // worklist of the cells k_multipoles_cells leaves to k_multipoles (NULL: all cells)
+    const uint32_t *corder;           // cells sorted by occupancy class (k_mp_order), dense cells last (NULL: identity, all cells to k_multipoles)
+    const uint32_t *nsmall;           // number of cells of up to NFM_LANE_MAX particles = start of the dense cells in `corder`
     const uint32_t *poff;             // first padded slot of each cell
     const float *sorted;              // the NF_PLANES sorted planes (hi offsets 0-2, lo remainders 4-6)
     uint32_t cap_pad;
@@ -47,24 +48,54 @@ struct MultipoleArgs {
 // from the sorted planes (hi + lo float32 = the double-precision offset to 2^-48; four particles per
 // 16-byte load and plane: cells are padded to 4 slots) and accumulates M[a,b,c] += (x^a y^b) z^c as
 // one DFMA per element into REGISTER accumulators -- no shared memory, no cross-lane reduction, no
-// atomics; 32 consecutive cells per warp.  165 accumulators do not fit in registers, so the basis is
-// cut by `a` into three slices (45 + 64 + 56 elements) done one after the other, each re-deriving
-// the particle's powers (+15 operations per slice and particle on top of the 165 + 45).  Lanes whose
-// cell is shorter than the warp's longest idle: fine at the paper's 30-100 per cell, which is why
-// cells above NFM_LANE_MAX go to k_multipoles (one CTA per cell) instead.
-#define NFM_LANE_MAX 256
+// atomics.  165 accumulators do not fit in registers, so the basis is cut into two slices of whole
+// (a, b) rows (88 + 77 elements) done one after the other, each re-reading the cell and re-deriving
+// the particle's offsets and powers: every extra slice costs a pass (measured: 3 slices +7 %, 7
+// slices 2.1x, although they allow twice the warps), so the slices are as large as 255 registers
+// hold.  A warp takes as long as its longest cell, so the lanes take their cells from a list sorted
+// by DESCENDING occupancy (k_mp_hist / k_mp_scan / k_mp_fill: a counting sort of the cell indices):
+// the 32 cells of a warp are equally long and the longest cells start first.  At 64 +- 8 per cell
+// this costs a little locality (+1 %); in the clustered configs, where neighbouring cells hold 5 and
+// 500, it is worth 20-25 %.  Cells above NFM_LANE_MAX go to k_multipoles (one CTA per cell).
+#define NFM_LANE_MAX 512
 
-template <int P, int A0, int A1>
+// The basis is cut into SLICES of whole (a, b) rows, filled greedily in index order up to NFM_SLICE_CAP
+// accumulators; slice_of(a, b) and the slice bounds are compile-time, so every test below folds away.
+#define NFM_SLICE_CAP 90      // 2 slices (88 + 77 accumulators) at p = 8: 255 registers, no spills, 2 warps per scheduler
+template <int P> struct MpSlices {
+    int sid[P + 1][P + 1];     // slice of row (a, b)
+    int base[64], cnt[64];     // first basis index and element count of a slice
+    int amin[64], amax[64], smax[64];   // range of a, and the largest power of y and z (P - a - b + ... ) a slice needs
+    int n;
+    constexpr MpSlices() : sid{}, base{}, cnt{}, amin{}, amax{}, smax{}, n(0) {
+        int cur = 0, fill = 0, idx = 0;
+        base[0] = 0; amin[0] = 0;
+        for (int a = 0; a <= P; ++a)
+            for (int b = 0; b <= P - a; ++b) {
+                const int len = P - a - b + 1;
+                if (fill > 0 && fill + len > NFM_SLICE_CAP) { cnt[cur] = fill; ++cur; fill = 0; base[cur] = idx; amin[cur] = a; smax[cur] = 0; }
+                sid[a][b] = cur;
+                amax[cur] = a;
+                if (b > smax[cur]) smax[cur] = b;
+                if (len - 1 > smax[cur]) smax[cur] = len - 1;
+                fill += len; idx += len;
+            }
+        cnt[cur] = fill;
+        n = cur + 1;
+    }
+};
+
+template <int P, int SID>
 __device__ __forceinline__ void mp_slice(const MultipoleArgs &A, uint32_t p0, uint32_t n, double *__restrict__ out) {
-    constexpr int base0 = []() { int s = 0; for (int a = 0; a < A0; ++a) s += (P - a + 1) * (P - a + 2) / 2; return s; }();
-    constexpr int NT = []() { int s = 0; for (int a = A0; a <= A1; ++a) s += (P - a + 1) * (P - a + 2) / 2; return s; }();
+    constexpr MpSlices<P> SL{};
+    constexpr int base0 = SL.base[SID], NT = SL.cnt[SID], A0 = SL.amin[SID], A1 = SL.amax[SID], SMAX = SL.smax[SID];
     double acc[NT];
 #pragma unroll
     for (int k = 0; k < NT; ++k) acc[k] = 0.0;
     const float *hx = A.sorted, *hy = A.sorted + A.cap_pad, *hz = A.sorted + 2ull * A.cap_pad;
     const float *lx = A.sorted + 4ull * A.cap_pad, *ly = A.sorted + 5ull * A.cap_pad, *lz = A.sorted + 6ull * A.cap_pad;
-    // the next four particles are requested before the current four are used: with two warps per
-    // scheduler the load latency has to be covered by the lane's own arithmetic
+    // the next four particles are requested before the current four are used: the load latency has to
+    // be covered by the lane's own arithmetic
     float4 HX, HY, HZ, LX, LY, LZ, nHX, nHY, nHZ, nLX, nLY, nLZ;
     auto fetch = [&](uint32_t j, float4 &a0, float4 &a1, float4 &a2, float4 &a3, float4 &a4, float4 &a5) {
         a0 = __ldg(reinterpret_cast<const float4 *>(hx + p0 + j)); a1 = __ldg(reinterpret_cast<const float4 *>(hy + p0 + j));
@@ -81,43 +112,103 @@ __device__ __forceinline__ void mp_slice(const MultipoleArgs &A, uint32_t p0, ui
             auto pick = [k](const float4 &v) { return k == 0 ? v.x : (k == 1 ? v.y : (k == 2 ? v.z : v.w)); };   // selects, no local memory
             const double X = ((double)pick(HX) + (double)pick(LX)) * A.cellsz, Y = ((double)pick(HY) + (double)pick(LY)) * A.cellsz,
                          Z = ((double)pick(HZ) + (double)pick(LZ)) * A.cellsz;
-            double zp[P + 1];                                            // z^c by squaring: dependency depth 3 instead of P
-            zp[0] = 1.0;
-            if (P >= 1) zp[1] = Z;
+            // powers by squaring (dependency depth 3 instead of P): the products x^a y^b of the rows are
+            // independent of one another, so the FMAs of one row never wait for the previous row's multiply
+            double zp[P + 1], yp[P + 1], xp[P + 1];
+            zp[0] = 1.0; yp[0] = 1.0; xp[0] = 1.0;
+            if (P >= 1) { zp[1] = Z; yp[1] = Y; xp[1] = X; }
 #pragma unroll
-            for (int c = 2; c <= P; ++c) zp[c] = zp[c / 2] * zp[c - c / 2];
-            double mx = 1.0;
+            for (int c = 2; c <= SMAX; ++c) { zp[c] = zp[c / 2] * zp[c - c / 2]; yp[c] = yp[c / 2] * yp[c - c / 2]; }
 #pragma unroll
-            for (int a = 0; a < A0; ++a) mx *= X;
+            for (int c = 2; c <= A1; ++c) xp[c] = xp[c / 2] * xp[c - c / 2];
             int idx = 0;
 #pragma unroll
             for (int a = A0; a <= A1; ++a) {
-                double mxy = mx;
 #pragma unroll
                 for (int b = 0; b <= P - a; ++b) {
+                    if (SL.sid[a][b] != SID) continue;
+                    const double mxy = (a == 0) ? yp[b] : ((b == 0) ? xp[a] : xp[a] * yp[b]);
 #pragma unroll
                     for (int c = 0; c <= P - a - b; ++c) { acc[idx] = fma(mxy, zp[c], acc[idx]); ++idx; }    // M[a,b,c] += mxy * Zc[c]
-                    mxy *= Y;
                 }
-                mx *= X;
             }
         }
     }
 #pragma unroll
     for (int k = 0; k < NT; ++k) out[base0 + k] = acc[k];
 }
+template <int P, int SID>
+__device__ __forceinline__ void mp_all_slices(const MultipoleArgs &A, uint32_t p0, uint32_t n, double *__restrict__ out) {
+    constexpr MpSlices<P> SL{};
+    if constexpr (SID < SL.n) {
+        mp_slice<P, SID>(A, p0, n, out);
+        mp_all_slices<P, SID + 1>(A, p0, n, out);
+    }
+}
+
+// Counting sort of the cell indices by occupancy class: class NFM_LANE_MAX - n for cells of n <= NFM_LANE_MAX
+// particles (longest first), one last class for the denser ones.  hist[0 .. NFM_LANE_MAX + 1] per class, then its exclusive scan;
+// hist[NFM_LANE_MAX + 2] receives the start of the dense class (= the number of lane cells).  The order
+// within a class is whatever the atomics give: which lane computes a cell does not change its result.
+#define NFM_NCLASS (NFM_LANE_MAX + 2)
+__device__ __forceinline__ uint32_t mp_class(uint32_t n) { return n <= NFM_LANE_MAX ? NFM_LANE_MAX - n : NFM_LANE_MAX + 1u; }   // longest lane cells first
+__global__ void __launch_bounds__(256) k_mp_hist(int ncell, const uint32_t *__restrict__ offsets, uint32_t *__restrict__ hist) {
+    __shared__ uint32_t h[NFM_NCLASS];
+    for (int i = threadIdx.x; i < NFM_NCLASS; i += blockDim.x) h[i] = 0u;
+    __syncthreads();
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += gridDim.x * blockDim.x) atomicAdd(&h[mp_class(offsets[c + 1] - offsets[c])], 1u);
+    __syncthreads();
+    for (int i = threadIdx.x; i < NFM_NCLASS; i += blockDim.x) if (h[i]) atomicAdd(&hist[i], h[i]);
+}
+__global__ void __launch_bounds__(256) k_mp_scan(uint32_t *hist) {      // one block: exclusive scan of the NFM_NCLASS class counts in place
+    constexpr int PER = (NFM_NCLASS + 255) / 256;
+    __shared__ uint32_t part[256];
+    uint32_t v[PER], s = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { const int i = threadIdx.x * PER + k; v[k] = i < NFM_NCLASS ? hist[i] : 0u; s += v[k]; }
+    part[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) { uint32_t t = 0; for (int i = 0; i < 256; ++i) { const uint32_t x = part[i]; part[i] = t; t += x; } }
+    __syncthreads();
+    uint32_t e = part[threadIdx.x];
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int i = threadIdx.x * PER + k;
+        if (i < NFM_NCLASS) { hist[i] = e; if (i == NFM_NCLASS - 1) hist[NFM_NCLASS] = e; }
+        e += v[k];
+    }
+}
+#define NFM_FILL_ITEMS 8
+__global__ void __launch_bounds__(256) k_mp_fill(int ncell, const uint32_t *__restrict__ offsets, uint32_t *__restrict__ hist, uint32_t *__restrict__ order) {
+    __shared__ uint32_t h[NFM_NCLASS];
+    for (int i = threadIdx.x; i < NFM_NCLASS; i += blockDim.x) h[i] = 0u;
+    __syncthreads();
+    uint32_t cls[NFM_FILL_ITEMS], rank[NFM_FILL_ITEMS];
+    const int c0 = blockIdx.x * (256 * NFM_FILL_ITEMS) + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < NFM_FILL_ITEMS; ++k) {
+        const int c = c0 + k * 256;
+        if (c < ncell) { cls[k] = mp_class(offsets[c + 1] - offsets[c]); rank[k] = atomicAdd(&h[cls[k]], 1u); }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < NFM_NCLASS; i += blockDim.x) if (h[i]) h[i] = atomicAdd(&hist[i], h[i]);      // the block's range in class i
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < NFM_FILL_ITEMS; ++k) {
+        const int c = c0 + k * 256;
+        if (c < ncell) order[h[cls[k]] + rank[k]] = (uint32_t)c;
+    }
+}
 
 template <int P>
-__global__ void __launch_bounds__(128) k_multipoles_cells(const MultipoleArgs A) {
-    const int cell = blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= A.ncell) return;
+__global__ void __launch_bounds__(128, 2) k_multipoles_cells(const MultipoleArgs A) {
+    const uint32_t w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= *A.nsmall) return;                           // the dense class: k_multipoles takes it
+    const int cell = (int)A.corder[w];
     const uint32_t n = A.offsets[cell + 1] - A.offsets[cell];
-    if (n > NFM_LANE_MAX) { A.dense[atomicAdd(A.ndense, 1u)] = (uint32_t)cell; return; }     // k_multipoles takes it
     const uint32_t p0 = A.poff[cell];
     double *out = A.M + (size_t)cell * A.cml;
-    mp_slice<P, 0, 0>(A, p0, n, out);
-    mp_slice<P, 1, 2>(A, p0, n, out);
-    mp_slice<P, 3, P>(A, p0, n, out);
+    mp_all_slices<P, 0>(A, p0, n, out);
 }
 
 // PMAX = compile-time bound of the order (8: the paper's choice; NFM_MAX_ORDER: any order)
@@ -149,9 +240,10 @@ __global__ void __launch_bounds__(160) k_multipoles(const MultipoleArgs A) {
     int ncw = nc;
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) ncw = max(ncw, __shfl_xor_sync(0xffffffffu, ncw, d));
-    const int nwork = A.dense ? (int)*A.ndense : A.ncell;
+    const int wstart = A.corder ? (int)*A.nsmall : 0;
+    const int nwork = A.ncell - wstart;
     for (int w = blockIdx.x; w < nwork; w += gridDim.x) {
-        const int cell = A.dense ? (int)A.dense[w] : w;
+        const int cell = A.corder ? (int)A.corder[wstart + w] : w;
         const uint32_t p0 = A.offsets[cell], p1 = A.offsets[cell + 1];
         double acc[PMAX + 1];
 #pragma unroll
@@ -216,12 +308,18 @@ nf_status nf_run_multipoles(nf_ctx *ctx, const float *d_pos, int order, double *
     A.pos = d_pos; A.offsets = ctx->d_offsets; A.perm = ctx->d_perm_true; A.M = d_M;
     A.scale = ctx->prm.scale; A.cellsz = ctx->box / (double)ctx->cpd;
     A.ncell = (int)ctx->ncell; A.order = order; A.cml = (order + 3) * (order + 2) * (order + 1) / 6;
-    A.dense = nullptr; A.ndense = nullptr; A.poff = ctx->d_poff; A.sorted = ctx->d_sorted; A.cap_pad = (uint32_t)ctx->capPad;
+    A.corder = nullptr; A.nsmall = nullptr; A.poff = ctx->d_poff; A.sorted = ctx->d_sorted; A.cap_pad = (uint32_t)ctx->capPad;
     const int64_t want = ctx->ncell;
     const int grid = (int)(want < (int64_t)ctx->sm_count * 2048 ? want : (int64_t)ctx->sm_count * 2048);
     if (order == 8) {        // the paper's order: a lane per cell, then the cells too dense for that by the CTA-per-cell kernel
-        A.dense = ctx->d_tmp_perm; A.ndense = ctx->d_ctrl + 6;           // (d_tmp_perm is free once the binning is done)
-        NF_CUDA_OK(ctx, cudaMemsetAsync(A.ndense, 0, sizeof(uint32_t), st));
+        uint32_t *order = ctx->d_tmp_perm;                               // (d_tmp_perm is free once the binning is done)
+        uint32_t *hist = ctx->d_mp_hist;
+        NF_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, (NFM_NCLASS + 1) * sizeof(uint32_t), st));
+        const int hgrid = (int)(want / 256 + 1 < (int64_t)ctx->sm_count * 8 ? want / 256 + 1 : (int64_t)ctx->sm_count * 8);
+        k_mp_hist<<<hgrid, 256, 0, st>>>(A.ncell, A.offsets, hist); ctx->launches++;
+        k_mp_scan<<<1, 256, 0, st>>>(hist); ctx->launches++;
+        k_mp_fill<<<(uint32_t)((want + 256 * NFM_FILL_ITEMS - 1) / (256 * NFM_FILL_ITEMS)), 256, 0, st>>>(A.ncell, A.offsets, hist, order); ctx->launches++;
+        A.corder = order; A.nsmall = hist + NFM_NCLASS;
         k_multipoles_cells<8><<<(uint32_t)((want + 127) / 128), 128, 0, st>>>(A); ctx->launches++;
     }
     const int dgrid = order == 8 ? ctx->sm_count * 16 : grid;           // the dense cells only: their number is on the device
