@@ -242,7 +242,42 @@ __global__ void __launch_bounds__(256) k_rank_gather(const float *__restrict__ p
     if (s == lo) big_cells[atomicAdd(&ctrl[7], 1u)] = k;
 }
 
-// the long cells: one CTA per worklist entry strides over the cell's slots
+// the long cells up to NF_SORT_MAX particles: one CTA per worklist entry sorts the cell's arrival list
+// (input indices) in shared memory with a bitonic network -- n log^2 n / 2 compare-exchanges against the
+// n (n / chunk) log chunk probes of the chunk method below, which keeps only the cells beyond
+// NF_SORT_MAX (more than fit in shared memory).
+#define NF_SORT_MAX 32768
+__global__ void __launch_bounds__(256) k_sort_big(const float *__restrict__ pos, double scale, uint32_t cap_pad,
+                                                  const uint32_t *__restrict__ ctrl, const uint32_t *__restrict__ offsets,
+                                                  const uint32_t *__restrict__ poff, const uint32_t *__restrict__ tmp_perm,
+                                                  const uint32_t *__restrict__ big_cells, float *__restrict__ sorted,
+                                                  uint32_t *__restrict__ perm_true, uint32_t *__restrict__ perm_pad,
+                                                  uint32_t nmin, uint32_t nmax /* this launch: cells of nmin < n <= nmax (its shared memory holds nmax) */) {
+    extern __shared__ uint32_t sidx[];
+    const uint32_t nbig = ctrl[7];
+    for (uint32_t w = blockIdx.x; w < nbig; w += gridDim.x) {
+        const uint32_t k = big_cells[w];
+        const uint32_t lo = poff[k], o0 = offsets[k], n = offsets[k + 1] - o0;
+        if (n <= nmin || n > nmax) continue;                                       // another launch, or k_rank_big
+        uint32_t P = 512;
+        while (P < n) P <<= 1;
+        __syncthreads();
+        for (uint32_t i = threadIdx.x; i < P; i += blockDim.x) sidx[i] = i < n ? tmp_perm[lo + i] : 0xffffffffu;
+        __syncthreads();
+        for (uint32_t kk = 2; kk <= P; kk <<= 1)
+            for (uint32_t j = kk >> 1; j > 0; j >>= 1) {
+                for (uint32_t t = threadIdx.x; t < (P >> 1); t += blockDim.x) {    // one compare-exchange per thread and step
+                    const uint32_t i = ((t & ~(j - 1u)) << 1) | (t & (j - 1u)), ixj = i | j;
+                    const uint32_t a = sidx[i], b = sidx[ixj];
+                    if ((a > b) == ((i & kk) == 0u)) { sidx[i] = b; sidx[ixj] = a; }
+                }
+                __syncthreads();
+            }
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) nf_place(pos, scale, cap_pad, sorted, perm_true, perm_pad, lo, o0, i, sidx[i]);
+    }
+}
+
+// the cells beyond NF_SORT_MAX: one CTA per worklist entry strides over the cell's slots
 __global__ void __launch_bounds__(256) k_rank_big(const float *__restrict__ pos, double scale, uint32_t cap_pad,
                                                   const uint32_t *__restrict__ ctrl, const uint32_t *__restrict__ offsets,
                                                   const uint32_t *__restrict__ poff, const uint32_t *__restrict__ chunk_sorted,
@@ -252,6 +287,7 @@ __global__ void __launch_bounds__(256) k_rank_big(const float *__restrict__ pos,
     for (uint32_t w = blockIdx.x; w < nbig; w += gridDim.x) {
         const uint32_t k = big_cells[w];
         const uint32_t lo = poff[k], o0 = offsets[k], n = offsets[k + 1] - o0;
+        if (n <= NF_SORT_MAX) continue;                                            // k_sort_big did it
         for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
             const uint32_t me = chunk_sorted[lo + i];
             uint32_t rank = i % NF_RANK_CHUNK;                                     // its place in its own sorted chunk
@@ -287,6 +323,12 @@ static nf_status binner_finish(nf_ctx *ctx, const float *d_pos, int64_t N, cudaS
                                                                    ctx->d_offsets, ctx->d_poff, ctx->d_tmp_perm, ctx->d_sorted,
                                                                    ctx->d_perm_true, ctx->d_perm_pad, ctx->d_chunk_sorted, ctx->d_key); ctx->launches++;
     // (d_key is free after the scatter: it holds the worklist of long cells, at most N / NF_RANK_CHUNK entries)
+    // two launches: the many cells of up to 8192 particles at 32 KB of shared memory (6 CTAs per SM), the few up to NF_SORT_MAX at 128 KB
+    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_sort_big, cudaFuncAttributeMaxDynamicSharedMemorySize, NF_SORT_MAX * 4));
+    k_sort_big<<<ctx->sm_count * 6, 256, 8192 * 4, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
+                                                        ctx->d_tmp_perm, ctx->d_key, ctx->d_sorted, ctx->d_perm_true, ctx->d_perm_pad, NF_RANK_CHUNK, 8192u); ctx->launches++;
+    k_sort_big<<<ctx->sm_count, 256, NF_SORT_MAX * 4, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
+                                                           ctx->d_tmp_perm, ctx->d_key, ctx->d_sorted, ctx->d_perm_true, ctx->d_perm_pad, 8192u, NF_SORT_MAX); ctx->launches++;
     k_rank_big<<<ctx->sm_count * 8, 256, 0, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
                                                   ctx->d_chunk_sorted, ctx->d_key, ctx->d_sorted, ctx->d_perm_true, ctx->d_perm_pad); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());

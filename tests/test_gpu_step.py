@@ -232,3 +232,39 @@ def test_rebin_without_a_binning_and_with_another_count(torch_cuda, NF, oracle_m
         nf.rebin(half)
         g = nf.debug_cells()
         assert np.array_equal(g["offsets"].astype(np.int64), o2) and np.array_equal(g["perm"].astype(np.int64), r2)
+
+
+def test_long_cells_in_every_rank_regime(torch_cuda, NF, oracle_mod):
+    """A3's stable order (ascending input index within a cell) for cells of every size class of the
+    binner: up to one 256-slot chunk (rank by counting), up to 8192 and up to 32768 (bitonic sort in
+    shared memory, two launches), beyond that (sorted chunks + binary searches) -- input order shuffled,
+    bit-exact against the oracle's counting sort; then the same through nf_rebin after a small drift."""
+    torch = torch_cuda
+    rng = np.random.default_rng(21)
+    cpd = 5
+    sizes = {(0, 0, 0): 40000, (1, 2, 3): 33000, (2, 2, 2): 20000, (3, 1, 0): 8192, (4, 4, 4): 8193, (0, 3, 1): 3000, (2, 0, 4): 257,
+             (1, 1, 1): 256, (3, 3, 3): 100, (4, 0, 2): 1}
+    parts = [((np.array(c) + rng.random((n, 3))) / cpd) for c, n in sizes.items()]
+    pos = np.concatenate(parts)
+    pos = pos[rng.permutation(len(pos))].astype(np.float32)
+    pos[pos >= 1.0] = 0.0
+    d = torch.from_numpy(pos).cuda()
+    with NF(cpd, 2, 0.002, 1.0) as nf:
+        nf.bin(d)
+        cell, off = oracle_mod.bin_particles(pos, cpd)
+        offsets, order = oracle_mod.cell_lists(cell, cpd)
+        g = nf.debug_cells()
+        assert np.array_equal(g["offsets"].astype(np.int64), offsets)
+        assert np.array_equal(g["perm"].astype(np.int64), order)
+        real = (g["sorted_key"] & 0x80000000) == 0
+        assert np.array_equal(g["sorted_key"][real].astype(np.int64), cell[order])
+        assert np.all(np.abs(g["sorted_xyz"][real] - off[order] * cpd) <= 1e-6)
+        moved = pos.copy()
+        moved[::7] = np.mod(moved[::7].astype(np.float64) + 0.03, 1.0).astype(np.float32)
+        moved[moved >= 1.0] = 0.0
+        d.copy_(torch.from_numpy(moved))
+        nf.rebin(d)
+        c2, _ = oracle_mod.bin_particles(moved, cpd)
+        o2, r2 = oracle_mod.cell_lists(c2, cpd)
+        g = nf.debug_cells()
+        assert np.array_equal(g["offsets"].astype(np.int64), o2) and np.array_equal(g["perm"].astype(np.int64), r2)
