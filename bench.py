@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- headline benchmark of the B200 near-field path (contract: task prompt, section 4).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4|all] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1..5] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (A1..A6: bin, scan, scatter, schedule, interact,
 un-permute) over one synthetic particle set.  Default workload: BASELINE.json configs[3]
@@ -14,7 +14,7 @@ nf_accel_host with pinned HOST buffers (H2D + D2H inside the timed region);
 ``roofline`` = FMA-pipe issue roofline of the interaction kernel (DESIGN.md "Roofline");
 ``cpu_baseline`` = the oracle timed on the host cores on a bounded sample.
 ``--impl reference`` times the oracle (there is no other reference implementation).
-``--config all`` measures configs 1, 2, 3, 5 as well and adds them under ``per_config`` (config 4
+``--config all`` (the default) measures configs 1, 2, 3, 5 as well and adds them under ``per_config`` (config 4
 stays the headline of the line).
 Multi-GPU (N > 1): the path shards: ONE particle set is cut into pair-balanced
 x slabs, one range per rank; a step = halo exchange of the R ghost slabs (isend/irecv over NCCL) +
@@ -508,16 +508,17 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="4", help="BASELINE.json config number 1..5 (default 4: CPD 135, N 157M), or 'all': "
-                                                  "config 4 as the headline plus the others under per_config")
+    ap.add_argument("--config", default="all", help="'all' (default): BASELINE.json config 4 (CPD 135, N 157M) as the headline of the line plus "
+                                                    "configs 1, 2, 3, 5 under per_config; or one config number 1..5")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target pair-loop time of the oracle for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--neighbours", action="store_true", help="also time nf_bin / nf_multipoles / nf_taylor_accel / nf_kick_drift at the workload")
-    ap.add_argument("--parallel", default="slabs", choices=["slabs", "replicas"],
+    ap.add_argument("--parallel", default=None, choices=["slabs", "replicas"],
                     help="N > 1: ONE particle set cut into x slabs with an R-slab halo exchange per step (default; strong "
-                         "scaling; paper_2110_11392_b200/slabs.py), or independent replicas (weak scaling)")
+                         "scaling; paper_2110_11392_b200/slabs.py), or independent replicas (weak scaling).  Given explicitly, "
+                         "'slabs' also runs the sharded code path on one GPU (one range, no ghosts)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print(f"note: --warmup {args.warmup} < 3 breaks the timing rules", file=sys.stderr)
@@ -528,7 +529,7 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     want_all = args.config == "all"
     k_main = 4 if want_all else int(args.config)
-    slabs_mode = world > 1 and args.parallel == "slabs"
+    slabs_mode = (world > 1 and args.parallel != "replicas") or args.parallel == "slabs"
 
     # ------------------------------------------------------------------ reference arm = the oracle
     if args.impl == "reference":
