@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(256) k_rank_gather(const float *__restrict__ p
 // n (n / chunk) log chunk probes of the chunk method below, which keeps only the cells beyond
 // NF_SORT_MAX (more than fit in shared memory).
 #define NF_SORT_MAX 32768
-__global__ void __launch_bounds__(256) k_sort_big(const float *__restrict__ pos, double scale, uint32_t cap_pad,
+__global__ void __launch_bounds__(1024) k_sort_big(const float *__restrict__ pos, double scale, uint32_t cap_pad,
                                                   const uint32_t *__restrict__ ctrl, const uint32_t *__restrict__ offsets,
                                                   const uint32_t *__restrict__ poff, const uint32_t *__restrict__ tmp_perm,
                                                   const uint32_t *__restrict__ big_cells, float *__restrict__ sorted,
@@ -327,7 +327,7 @@ static nf_status binner_finish(nf_ctx *ctx, const float *d_pos, int64_t N, cudaS
     NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_sort_big, cudaFuncAttributeMaxDynamicSharedMemorySize, NF_SORT_MAX * 4));
     k_sort_big<<<ctx->sm_count * 6, 256, 8192 * 4, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
                                                         ctx->d_tmp_perm, ctx->d_key, ctx->d_sorted, ctx->d_perm_true, ctx->d_perm_pad, NF_RANK_CHUNK, 8192u); ctx->launches++;
-    k_sort_big<<<ctx->sm_count, 256, NF_SORT_MAX * 4, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
+    k_sort_big<<<ctx->sm_count, 1024, NF_SORT_MAX * 4, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
                                                            ctx->d_tmp_perm, ctx->d_key, ctx->d_sorted, ctx->d_perm_true, ctx->d_perm_pad, 8192u, NF_SORT_MAX); ctx->launches++;
     k_rank_big<<<ctx->sm_count * 8, 256, 0, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
                                                   ctx->d_chunk_sorted, ctx->d_key, ctx->d_sorted, ctx->d_perm_true, ctx->d_perm_pad); ctx->launches++;
