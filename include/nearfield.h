@@ -24,7 +24,12 @@
  *     writes d_pos / h_pos.  The context owns all scratch (grow-only).
  *   - All device work of nf_accel is enqueued on `cuda_stream` (a cudaStream_t passed as
  *     void*; NULL = the legacy default stream); the call returns without synchronising.
- *     One context = one call in flight.
+ *     One stream at a time per context: the context's scratch is shared by its calls, so a
+ *     call on another stream than the previous call's is ordered after it (an event on the
+ *     previous stream, waited on by the new one) -- two calls on one context never overlap;
+ *     use one context per stream for concurrency.  A stream handed to a call must stay
+ *     valid until the next call on the context or nf_sync.  Calls are not thread-safe per
+ *     context (one host thread at a time).
  *   - Every function returns an nf_status and never throws or aborts; nf_last_error gives
  *     the text of the last failure on that context.
  *   - There is no CPU fallback: without a CUDA device nf_create fails with NF_ECUDA.
@@ -319,6 +324,11 @@ nf_status nf_debug_cells(nf_ctx *ctx, const uint32_t **d_offsets, const uint32_t
 /* nf_close_radius -- the close-pair radius (cell units) the last nf_accel used; 0 = none
  * (see option "rc_cells").  Synchronises. */
 nf_status nf_close_radius(nf_ctx *ctx, double *h_rc_cells);
+
+/* nf_bounds_checked -- 1 if this library is the -DNF_DEBUG_BOUNDS build (every index the kernels derive
+ * is checked against the bound of its array; nf_sync returns NF_ECUDA "bounds check <code> failed" on a
+ * violation), 0 for the product build.  No context needed. */
+int nf_bounds_checked(void);
 
 /* nf_launch_count -- number of CUDA kernels this context has launched since nf_create
  * (memsets and copies are not counted).  bench.py reports the difference over its timed region. */

@@ -23,7 +23,7 @@ SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", 
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
            "nf_interaction_count", "nf_debug_read", "nf_launch_count", "nf_close_radius",
            "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles", "nf_kick_drift", "nf_timestep_ratio", "nf_taylor_accel",
-           "nf_debug_delivered_pairs", "nf_bin", "nf_rebin", "nf_unbin", "nf_cell_histogram", "nf_slab_pairs", "nf_select_slabs"]
+           "nf_debug_delivered_pairs", "nf_bounds_checked", "nf_bin", "nf_rebin", "nf_unbin", "nf_cell_histogram", "nf_slab_pairs", "nf_select_slabs"]
 
 
 class NearFieldError(RuntimeError):
@@ -103,6 +103,8 @@ def load_library() -> ctypes.CDLL:
     L.nf_select_slabs.argtypes = [vp, vp, i64, i32, i32, vp, ctypes.POINTER(i64), vp]
     L.nf_close_radius.restype = i32
     L.nf_close_radius.argtypes = [vp, ctypes.POINTER(dbl)]
+    L.nf_bounds_checked.restype = i32
+    L.nf_bounds_checked.argtypes = []
     L.nf_launch_count.restype = i32
     L.nf_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     L.nf_debug_read.restype = i32
@@ -111,6 +113,11 @@ def load_library() -> ctypes.CDLL:
 
 
 _L = load_library()
+
+
+def bounds_checked() -> bool:
+    """nf_bounds_checked: is the loaded library the -DNF_DEBUG_BOUNDS build?"""
+    return bool(_L.nf_bounds_checked())
 
 
 class NearField:

@@ -93,6 +93,29 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_debug_library(out: str, verbose: bool = False) -> str:
+    """The -DNF_DEBUG_BOUNDS build of the product library (csrc/nf_common.cuh: every derived index is checked
+    against the bound of its array; nf_sync reports a violation), written to ``out`` -- never over the
+    in-tree library.  tests/test_gpu_debug_bounds.py runs the small parity cases under it."""
+    nvcc = os.environ.get("NVCC", "nvcc")
+    objdir = out + ".obj"
+    os.makedirs(objdir, exist_ok=True)
+
+    def one(src: str) -> str:
+        obj = os.path.join(objdir, src.replace(os.sep, "_") + ".o")
+        cmd = [nvcc, *NVCC_FLAGS, "-DNF_DEBUG_BOUNDS", "-c", "-o", obj, os.path.join(CSRC, src)]
+        if verbose:
+            cmd.insert(1, "-Xptxas=-v")
+        subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(8, len(SOURCES))) as ex:
+        objs = list(ex.map(one, SOURCES))
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", out, *objs],
+                   check=True, stdout=sys.stderr, stderr=sys.stderr)
+    return out
+
+
 def ensure_built() -> str:
     """Make sure the in-tree libraries exist and are not older than their sources (a fresh checkout
     has none: they are not tracked).  A build step, not a fallback: without nvcc a stale or missing
@@ -103,4 +126,7 @@ def ensure_built() -> str:
 
 
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--debug-bounds" in sys.argv:
+        print(build_debug_library(sys.argv[sys.argv.index("--debug-bounds") + 1], verbose="-v" in sys.argv))
+    else:
+        print(build_library(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -83,6 +83,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
         if (cudaEventCreate(&c->ev[i]) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaEventCreate failed"); return fail(NF_ECUDA); }
     if (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
         cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaStreamCreate failed"); return fail(NF_ECUDA); }
+    if (cudaEventCreateWithFlags(&c->ev_order, cudaEventDisableTiming) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaEventCreate failed"); return fail(NF_ECUDA); }
     for (int i = 0; i < NF_HOST_CHUNKS; ++i)
         if (cudaEventCreateWithFlags(&c->ev_chunk[i], cudaEventDisableTiming) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaEventCreate failed"); return fail(NF_ECUDA); }
     rc = nf_interact_setup(c);
@@ -101,11 +102,20 @@ extern "C" nf_status nf_destroy(nf_ctx *c) {
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < NF_HOST_CHUNKS; ++i) if (c->ev_chunk[i]) cudaEventDestroy(c->ev_chunk[i]);
+    if (c->ev_order) cudaEventDestroy(c->ev_order);
     if (c->own_stream) cudaStreamDestroy(c->own_stream);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     cudaGetLastError();
     delete c;
     return NF_OK;
+}
+
+extern "C" int nf_bounds_checked(void) {
+#ifdef NF_DEBUG_BOUNDS
+    return 1;
+#else
+    return 0;
+#endif
 }
 
 extern "C" const char *nf_last_error(const nf_ctx *c) { return c ? c->err : g_static_err; }
@@ -131,6 +141,17 @@ extern "C" nf_status nf_set_option(nf_ctx *c, const char *name, double v) {
     else if (!strcmp(name, "heavy_first")) c->opt_heavy_first = iv;
     else { snprintf(c->err, sizeof c->err, "nf_set_option: unknown option '%s'", name); return NF_EINVAL; }
     return NF_OK;
+}
+
+// One stream at a time per context: the scratch of a context is shared by its calls.  When a call
+// arrives on another stream than the previous one, its work is ordered after that call's (an event on
+// the previous stream, waited on by the new one) -- calls on different streams never overlap on one context.
+static void enter_stream(nf_ctx *c, cudaStream_t st) {
+    if (c->have_last && c->last_stream != st) {
+        if (cudaEventRecord(c->ev_order, c->last_stream) == cudaSuccess) cudaStreamWaitEvent(st, c->ev_order, 0);
+        else cudaGetLastError();
+    }
+    c->last_stream = st; c->have_last = 1;
 }
 
 static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
@@ -180,7 +201,7 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
 static nf_status bin_for(nf_ctx *c, const float *d_pos, int64_t N, cudaStream_t st) {
     nf_status rc = ensure_scratch(c, N);
     if (rc != NF_OK) return rc;
-    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    enter_stream(c, st); c->lastN = N;
     if (c->bin_pinned && c->bin_pos == d_pos && c->bin_N == N) return NF_OK;
     c->bin_pinned = 0; c->have_sched = 0; c->bin_valid = 0;
     rc = nf_run_binner(c, d_pos, N, st);
@@ -229,7 +250,7 @@ extern "C" nf_status nf_rebin(nf_ctx *c, const float *d_pos, int64_t N, void *cu
         }
         c->capRebin = c->capN;
     }
-    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    enter_stream(c, st); c->lastN = N;
     c->bin_pinned = 0; c->have_sched = 0; c->bin_valid = 0;
     nf_status rc = nf_run_rebin(c, d_pos, N, st);
     if (rc != NF_OK) return rc;
@@ -266,7 +287,7 @@ extern "C" nf_status nf_cell_histogram(nf_ctx *c, const float *d_pos, int64_t N,
     c->err[0] = 0;
     if (N < 0 || !d_counts || (N > 0 && !d_pos) || N >= 2147483647ll) { snprintf(c->err, sizeof c->err, "nf_cell_histogram: bad argument (N=%lld)", (long long)N); return NF_EINVAL; }
     NF_CUDA_OK(c, cudaSetDevice(c->device));
-    c->last_stream = (cudaStream_t)cuda_stream; c->have_last = 1;
+    enter_stream(c, (cudaStream_t)cuda_stream);
     return nf_run_cell_histogram(c, d_pos, N, d_counts, (cudaStream_t)cuda_stream);
 }
 
@@ -292,7 +313,7 @@ extern "C" nf_status nf_select_slabs(nf_ctx *c, const float *d_pos, int64_t N, i
     NF_CUDA_OK(c, cudaSetDevice(c->device));
     nf_status rc = ensure_scratch(c, N);
     if (rc != NF_OK) return rc;
-    c->last_stream = st; c->have_last = 1; c->have_sched = 0;      // (the block scan reuses ctrl[1])
+    enter_stream(c, st); c->have_sched = 0;      // (the block scan reuses ctrl[1])
     rc = nf_run_select_slabs(c, d_pos, N, x0, nx, d_out, c->d_key, st);
     if (rc != NF_OK) return rc;
     uint32_t tot = 0;
@@ -442,8 +463,9 @@ extern "C" nf_status nf_sync(nf_ctx *c) {
     if (!c) return NF_EINVAL;
     if (!c->have_last) return NF_OK;
     NF_CUDA_OK(c, cudaStreamSynchronize(c->last_stream));
-    uint32_t ctrl[4];
+    uint32_t ctrl[16];
     NF_CUDA_OK(c, cudaMemcpy(ctrl, c->d_ctrl, sizeof ctrl, cudaMemcpyDeviceToHost));
+    if (ctrl[8]) { snprintf(c->err, sizeof c->err, "bounds check %u failed in a kernel (NF_DEBUG_BOUNDS build)", ctrl[8]); return NF_ECUDA; }
     if (ctrl[2]) { snprintf(c->err, sizeof c->err, "nf_accel: a position was NaN or infinite"); return NF_EPOS; }
     return NF_OK;
 }
@@ -469,7 +491,7 @@ extern "C" nf_status nf_accel_host(nf_ctx *c, const float *h_pos, int64_t N, flo
     c->err[0] = 0;
     nf_status rc = ensure_scratch(c, N);
     if (rc != NF_OK) return rc;
-    c->last_stream = st; c->lastN = N; c->have_last = 1;
+    enter_stream(c, st); c->lastN = N;
     c->bin_pinned = 0; c->have_sched = 0; c->bin_valid = 0;
     rc = nf_run_binner_host(c, h_pos, c->d_pos_buf, N, st);
     if (rc != NF_OK) return rc;

@@ -179,11 +179,12 @@ nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out
 // ------------------------------------------------------------------------------ A3
 __global__ void __launch_bounds__(256) k_scatter(uint32_t N, const uint32_t *__restrict__ key, const uint32_t *__restrict__ arr,
                                                  const uint32_t *__restrict__ counts, const uint32_t *__restrict__ poff,
-                                                 uint32_t *__restrict__ tmp_perm, uint32_t *__restrict__ skey) {
+                                                 uint32_t *__restrict__ tmp_perm, uint32_t *__restrict__ skey, const uint32_t *__restrict__ ctrl) {
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     uint32_t k = key[i], r = arr[i];
     uint32_t slot = poff[k] + r;
+    NF_CHECK(ctrl, slot < ctrl[3] && r < counts[k], 16);
     tmp_perm[slot] = i;
     skey[slot] = k;
     if (r == 0) {
@@ -237,6 +238,7 @@ __global__ void __launch_bounds__(256) k_rank_gather(const float *__restrict__ p
     const uint32_t c1 = (c0 + NF_RANK_CHUNK < lo + n) ? c0 + NF_RANK_CHUNK : lo + n;
     uint32_t rank = 0;
     for (uint32_t t = c0; t < c1; ++t) rank += (tmp_perm[t] < me) ? 1u : 0u;
+    NF_CHECK(ctrl, rank < c1 - c0 && me < 0x7fffffffu, 17);
     if (n <= NF_RANK_CHUNK) { nf_place(pos, scale, cap_pad, sorted, perm_true, perm_pad, lo, o0, rank, me); return; }
     chunk_sorted[c0 + rank] = me;
     if (s == lo) big_cells[atomicAdd(&ctrl[7], 1u)] = k;
@@ -273,7 +275,10 @@ __global__ void __launch_bounds__(1024) k_sort_big(const float *__restrict__ pos
                 }
                 __syncthreads();
             }
-        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) nf_place(pos, scale, cap_pad, sorted, perm_true, perm_pad, lo, o0, i, sidx[i]);
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+            NF_CHECK(ctrl, sidx[i] != 0xffffffffu && (i == 0 || sidx[i - 1] < sidx[i]), 19);
+            nf_place(pos, scale, cap_pad, sorted, perm_true, perm_pad, lo, o0, i, sidx[i]);
+        }
     }
 }
 
@@ -301,6 +306,7 @@ __global__ void __launch_bounds__(256) k_rank_big(const float *__restrict__ pos,
                 }
                 rank += a - first;
             }
+            NF_CHECK(ctrl, rank < n, 20);
             nf_place(pos, scale, cap_pad, sorted, perm_true, perm_pad, lo, o0, rank, me);
         }
     }
@@ -314,7 +320,7 @@ static nf_status binner_finish(nf_ctx *ctx, const float *d_pos, int64_t N, cudaS
     if (rc != NF_OK) return rc;
     if (ctx->opt_stage_timing) cudaEventRecord(ctx->ev[2], st);
     uint32_t *skey = (uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
-    k_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_poff, ctx->d_tmp_perm, skey); ctx->launches++;
+    k_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, ctx->d_key, ctx->d_arr, ctx->d_counts, ctx->d_poff, ctx->d_tmp_perm, skey, ctx->d_ctrl); ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());
     // upper bound of the padded slot count: N + ncell (+8 slack), known on the host
     uint64_t bound = (uint64_t)N + (uint64_t)(NF_CELL_PAD - 1) * (uint64_t)ctx->ncell + 8;

@@ -91,7 +91,7 @@ struct nf_ctx {
     uint32_t *d_pair_slot;       // sink pair i (sink-order slots 2i, 2i+1) -> padded slot of its first sink (A4)
     NfBlockDesc *d_blk;
     uint32_t *d_ctrl;            // [0] work counter  [1] number of blocks  [2] bad-position flag  [3] npad
-                                 // [4] sink-order slot count
+                                 // [4] sink-order slot count  [8] NF_DEBUG_BOUNDS: code of a failed bounds check
                                  // [5] insert-list tail (nf_rebin)  [6] dense-cell count (nf_multipoles)  [7] long-cell count (rank)
                                  // [16..79] cost histogram  [96..98] float rc^2, rc, rc^-3  [100..101] u64 sum n_c^2  [104] work counter of nf_accel_f64
     unsigned long long *d_pairs;
@@ -102,6 +102,7 @@ struct nf_ctx {
     cudaStream_t own_stream;
     cudaStream_t copy_stream;    // nf_accel_host: H2D ranges, each followed by A1 on the compute stream
     cudaEvent_t ev_chunk[NF_HOST_CHUNKS];
+    cudaEvent_t ev_order;        // orders a call after the previous one when the stream changes
     // state of the last call
     cudaStream_t last_stream;
     int64_t lastN;
@@ -114,6 +115,17 @@ struct nf_ctx {
     cudaEvent_t ev[8];
     char err[512];
 };
+
+// -DNF_DEBUG_BOUNDS build (python -m paper_2110_11392_b200.build --debug-bounds <out.so>): every index the
+// kernels derive from the offset tables, the ring cursor and the permutations is checked against the
+// bound of the array it addresses; a violation records its code in ctrl[8] (largest code wins) and
+// nf_sync reports it as NF_ECUDA.  tests/test_gpu_debug_bounds.py runs the small parity cases under it
+// (compute-sanitizer is not available on this pool).  Compiled out of the product library.
+#ifdef NF_DEBUG_BOUNDS
+#define NF_CHECK(ctrl, cond, code) do { if (!(cond)) atomicMax(const_cast<uint32_t *>(ctrl) + 8, (uint32_t)(code)); } while (0)
+#else
+#define NF_CHECK(ctrl, cond, code) do { } while (0)
+#endif
 
 #define NF_CUDA_OK(ctx, call)                                                                   \
     do {                                                                                        \

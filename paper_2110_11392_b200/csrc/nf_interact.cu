@@ -86,7 +86,10 @@ __global__ void __launch_bounds__(256) k_pair_slots(uint32_t cap_pad, const uint
     if (s >= ctrl[3]) return;
     const uint32_t k = skey[s] & ~NF_PAD_FLAG;
     const uint32_t t = s - poff[k];
-    if (t < offsets[k + 1] - offsets[k]) pair_slot[(poff2[k] + t) >> 1] = s;
+    if (t < offsets[k + 1] - offsets[k]) {
+        NF_CHECK(ctrl, ((poff2[k] + t) >> 1) < (ctrl[4] + 1u) / 2u && ((poff2[k] + t) >> 1) < cap_pad / 2u + 8u, 18);
+        pair_slot[(poff2[k] + t) >> 1] = s;
+    }
 }
 
 __global__ void __launch_bounds__(256) k_col_blocks(int ncol, int cpd, int x0, int nx, const uint32_t *__restrict__ poff, uint32_t *__restrict__ col_nblk) {
@@ -272,6 +275,7 @@ struct InteractArgs {
     const float *sx, *sy, *sz, *lx, *ly, *lz;   // hi planes (staged into shared memory) and lo planes (close_scan only)
     const uint32_t *skey, *poff, *perm_pad, *order;
     const uint32_t *pair_slot;                  // sink pair -> padded slot of its first sink
+    uint32_t n_part;                            // particles of the call (NF_DEBUG_BOUNDS: bound of the un-permute)
     const NfBlockDesc *blk;
     uint32_t *ctrl;
     const float *dyn;        // [0] rc^2 (cell units^2; 0 = no close-pair radius, use the min form)  [1] rc  [2] rc^-3
@@ -303,6 +307,7 @@ struct InteractArgs {
 struct CloseArgs {
     const float *sx, *sy, *sz;   // hi planes (global; the sink's own offsets)
     const float *lx, *ly, *lz;   // lo planes
+    const uint32_t *ctrl;
     double eps;                // eps_s in cell units (0: no softening)
     double soft2;              // eps_p^2 in cell units (Plummer) or 0
     float addend;              // the loop's r^2 addend
@@ -351,6 +356,7 @@ __device__ __noinline__ void close_scan(const CloseArgs &K, const float *xs, con
                 // what the hot loop added for this pair (f clamped to fmax)
                 cx -= (double)fmax * (double)dxf; cy -= (double)fmax * (double)dyf; cz -= (double)fmax * (double)dzf;
                 const uint32_t q = g_lo + (uint32_t)s;        // padding never gets here (x = +BIG)
+                NF_CHECK(K.ctrl, q < K.ctrl[3] && s >= 0 && s < NF_TILE, 8);
                 if (q == sink_slot) continue;                 // the particle itself: F(0) = 0
                 const double dx = (((double)xs[s] + (double)K.lx[q]) - opx) + (double)a;
                 const double dy = (((double)ys[s] + (double)K.ly[q]) - opy) + (double)b;
@@ -575,6 +581,8 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
         uint64_t *fb = &full_bar[pstage];
         auto emit = [&](int flags, int a, int b, int zu0, int nc, uint32_t tabval, uint32_t g_lo, int g_cnt, uint32_t col, uint32_t s0, uint32_t cnt) {
             S.tab[lane] = tabval;
+            NF_CHECK(A.ctrl, g_cnt >= 0 && g_cnt <= NF_TILE && (g_lo & 3u) == 0u && g_lo + (uint32_t)g_cnt <= A.ctrl[3] + 8u, 1);
+            NF_CHECK(A.ctrl, tabval <= (uint32_t)g_cnt, 2);
             if (lane == 0) {
                 StageHdr h;
                 h.flags = flags; h.a = a; h.b = b; h.zu0 = zu0; h.nc = nc; h.g_lo = g_lo; h.g_cnt = g_cnt;
@@ -657,7 +665,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
     const float rc2 = A.dyn[3];
     const float fmax = A.dyn[2];
     CloseArgs K;
-    K.sx = A.sx; K.sy = A.sy; K.sz = A.sz; K.lx = A.lx; K.ly = A.ly; K.lz = A.lz; K.eps = A.close_eps;
+    K.ctrl = A.ctrl; K.sx = A.sx; K.sy = A.sy; K.sz = A.sz; K.lx = A.lx; K.ly = A.ly; K.lz = A.lz; K.eps = A.close_eps;
     K.law = LAW; K.addend = A.addend; K.soft2 = (LAW == NF_SOFT_PLUMMER) ? (double)A.addend : 0.0;
     const int tid_s = (int)threadIdx.x * kS;           // this thread's first column of close_corr / tot
     float px[kS], py[kS], pz[kS];
@@ -708,9 +716,12 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
         if (flags & NF_F_NEWBLOCK) {
             const uint32_t off = (uint32_t)(warp * 32 + lane) * kS;
             valid = off < S.hdr.cnt;
+            NF_CHECK(A.ctrl, ((S.hdr.s0 + (valid ? off : 0u)) >> 1) < (A.ctrl[4] + 1u) / 2u, 3);
             slot = A.pair_slot[(S.hdr.s0 + (valid ? off : 0u)) >> 1];
+            NF_CHECK(A.ctrl, slot + 1u < A.ctrl[3] && (slot & 1u) == 0u, 4);
             const int colbase = (int)S.hdr.col * cpd;
             zl = (int)(A.skey[slot] & ~NF_PAD_FLAG) - colbase;
+            NF_CHECK(A.ctrl, zl >= 0 && zl < cpd, 5);
 #pragma unroll
             for (int j = 0; j < kS; ++j) {
                 px[j] = valid ? A.sx[slot + j] : -NF_BIG;   // an idle lane sits at -BIG: contributes and receives exactly 0
@@ -762,6 +773,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                 const int cell = useA ? pcA : pcB;
                 const int lo = useA ? ploA : ploB;
                 const int dzc = cell - zl;
+                NF_CHECK(A.ctrl, !(useA || useB) || (lo >= 0 && n > 0 && (lo & 3) == 0 && (n & 3) == 0 && lo + n <= S.hdr.g_cnt), 6);
                 float xim[kS], zi[kS];
                 uint32_t bits[kS];
 #pragma unroll
@@ -841,6 +853,7 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
 #pragma unroll
                 for (int j = 0; j < kS; ++j) {
                     const uint32_t dst = A.perm_pad[slot + j];
+                    NF_CHECK(A.ctrl, dst == 0xffffffffu || dst < A.n_part, 7);
                     if (dst != 0xffffffffu) {
                         float *o = A.acc + (size_t)A.ostride * dst;
                         o[0] = (float)((double)A.kfac * ((double)tot[0][tid_s + j] + close_corr[0][tid_s + j]));
@@ -904,6 +917,7 @@ static void fill_interact_args(nf_ctx *ctx, const float *d_pos, float *d_out, in
     A.lx = ctx->d_sorted + 4ull * ctx->capPad; A.ly = ctx->d_sorted + 5ull * ctx->capPad; A.lz = ctx->d_sorted + 6ull * ctx->capPad;
     A.skey = (const uint32_t *)(ctx->d_sorted + 3ull * ctx->capPad);
     A.poff = ctx->d_poff; A.perm_pad = ctx->d_perm_pad; A.order = ctx->d_blk_order; A.blk = ctx->d_blk; A.pair_slot = ctx->d_pair_slot;
+    A.n_part = (uint32_t)ctx->lastN;
     A.ctrl = ctx->d_ctrl; A.dyn = (const float *)(ctx->d_ctrl + 96); A.acc = d_out; A.kfac = kfac; A.prm = ctx->prm;
     A.prm.kahan = ctx->opt_kahan;
     A.ostride = ostride;

@@ -332,6 +332,21 @@ def test_user_stream_and_stage_times(torch_cuda, NF):
         b = nf.accel(pos)
         torch.cuda.synchronize()
         assert torch.equal(a, b)
+        # one stream at a time per context: calls on alternating streams with no synchronisation in
+        # between are ordered by the library (they share the context's scratch) and give the same result
+        s2 = torch.cuda.Stream()
+        other = torch.from_numpy(W.uniform(cfg.N // 3, 17)).cuda()
+        torch.cuda.synchronize()
+        outs = []
+        for it in range(6):
+            stream = st if it % 2 == 0 else s2
+            with torch.cuda.stream(stream):
+                outs.append(nf.accel(pos if it % 3 else other, stream=stream))
+        torch.cuda.synchronize()
+        ref_other = nf.accel(other)
+        torch.cuda.synchronize()
+        for it, o in enumerate(outs):
+            assert torch.equal(o, a if it % 3 else ref_other), it
 
 
 # ----------------------------------------------------------------------------- full-size configs (sampled)
