@@ -403,6 +403,22 @@ def _neighbour_steps(nf, d_pos, d_acc, cfg, peaks_live, order: int = 8) -> dict:
     del M
     vel = torch.zeros_like(d_pos)
     res["kick_drift_ms"] = timed(lambda: nf.kick_drift(d_pos, vel, d_acc, 0.0, 0.0))
+    # nf_rebin after a drift of 0.05 cell rms per component (a few per cent of the particles change cell: PAPER.md:356
+    # "most particles stay in their cell") against the full sort above; the drift itself is not timed
+    vel = torch.randn_like(d_pos) * (0.05 * cfg.box / cfg.cpd)
+    nf.bin(d_pos)
+    ts = []
+    for _ in range(3):
+        nf.kick_drift(d_pos, vel, d_acc, 0.0, 1.0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        nf.rebin(d_pos)
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    res["rebin_ms_after_drift_0.05_cell"] = min(ts[1:])          # the first call allocates the insert list
+    del vel
     nf.unbin()
     dfma = peaks_live["dfma_lane_ops_per_s"]
     # algorithmic FP64 FMA-class operations per particle: multipoles cml FMAs + (p+1)(p+2)/2
