@@ -7,8 +7,9 @@
 // paper computes the multipoles in double: "double M[cml]").  cml = (p+3)(p+2)(p+1)/6
 // values per cell, index order = the (a, b, c) nesting of the paper's pseudo-code.
 //
-// Two mappings.  Order 8, cells of up to NFM_LANE_MAX particles: k_multipoles_cells, a lane per cell
-// (below).  Everything else (other orders; dense cells): k_multipoles, where the
+// Two mappings.  Order 8 (the paper's): k_multipoles_cells, a lane per cell -- or per 512-particle
+// chunk of a cell denser than NFM_LANE_MAX, whose partial sums k_mp_reduce adds (below).  The other
+// orders: k_multipoles, where the
 // BASIS is spread across threads and the particles of the cell stream past it: one CTA per
 // cell, 64 threads up to order 9 (160 above); thread t owns one (a, b) pair -- pairs sorted by
 // descending element count p-a-b+1, so that the first warp holds the long ones and the second
@@ -35,8 +36,6 @@ struct MultipoleArgs {
     double *M;
     double scale, cellsz;
     int ncell, order, cml;
-    const uint32_t *corder;           // cells sorted by occupancy class (k_mp_order), dense cells last (NULL: identity, all cells to k_multipoles)
-    const uint32_t *nsmall;           // number of cells of up to NFM_LANE_MAX particles = start of the dense cells in `corder`
     const uint32_t *poff;             // first padded slot of each cell
     const float *sorted;              // the NF_PLANES sorted planes (hi offsets 0-2, lo remainders 4-6)
     uint32_t cap_pad;
@@ -56,8 +55,8 @@ struct MultipoleArgs {
 // by DESCENDING occupancy (k_mp_hist / k_mp_scan / k_mp_fill: a counting sort of the cell indices):
 // the 32 cells of a warp are equally long and the longest cells start first.  At 64 +- 8 per cell
 // this costs a little locality (+1 %); in the clustered configs, where neighbouring cells hold 5 and
-// 500, it is worth 20-25 %.  Cells above NFM_LANE_MAX go to k_multipoles (one CTA per cell).
-#define NFM_LANE_MAX 512
+// 500, it is worth 20-25 %.  Cells above NFM_LANE_MAX are cut into chunks that are work items of their own.
+#define NFM_LANE_MAX 1024
 
 // The basis is cut into SLICES of whole (a, b) rows, filled greedily in index order up to NFM_SLICE_CAP
 // accumulators; slice_of(a, b) and the slice bounds are compile-time, so every test below folds away.
@@ -146,17 +145,34 @@ __device__ __forceinline__ void mp_all_slices(const MultipoleArgs &A, uint32_t p
     }
 }
 
-// Counting sort of the cell indices by occupancy class: class NFM_LANE_MAX - n for cells of n <= NFM_LANE_MAX
-// particles (longest first), one last class for the denser ones.  hist[0 .. NFM_LANE_MAX + 1] per class, then its exclusive scan;
-// hist[NFM_LANE_MAX + 2] receives the start of the dense class (= the number of lane cells).  The order
-// within a class is whatever the atomics give: which lane computes a cell does not change its result.
-#define NFM_NCLASS (NFM_LANE_MAX + 2)
-__device__ __forceinline__ uint32_t mp_class(uint32_t n) { return n <= NFM_LANE_MAX ? NFM_LANE_MAX - n : NFM_LANE_MAX + 1u; }   // longest lane cells first
+// The lane kernel's WORK ITEMS are cells of up to NFM_LANE_MAX particles and, for the denser cells of a
+// clustered state, CHUNKS of NFM_CHUNK consecutive particles of one cell; a chunk's result goes to a
+// partial buffer and k_mp_reduce adds a cell's partials in chunk order (a fixed order: deterministic).
+// The items are sorted by DESCENDING particle count (counting sort: class = NFM_LANE_MAX - count), so the
+// 32 items of a warp are equally long and the longest start first.  hist[0 .. NFM_NCLASS) per class, then
+// its exclusive scan (k_mp_scan), then the running cursors of k_mp_fill; hist[NFM_NCLASS] = number of items;
+// hist[NFM_CTR_CHUNK] / hist[NFM_CTR_DENSE] count the chunks and the dense cells.  The order within a class
+// is whatever the atomics give: which lane computes an item does not change its result.
+// A dense cell (n > NFM_LANE_MAX = 2 NFM_CHUNK) has ceil(n / NFM_CHUNK) <= 3 n / (2 NFM_LANE_MAX) chunks, so
+// all chunks of any input fit the partial buffer (the binner's chunk scratch: 4 capPad bytes >= N / 330 chunks).
+#define NFM_CHUNK 512
+#define NFM_NCLASS (NFM_LANE_MAX + 1)
+#define NFM_CTR_CHUNK (NFM_NCLASS + 1)
+#define NFM_CTR_DENSE (NFM_NCLASS + 2)
+static_assert(NFM_LANE_MAX == 2 * NFM_CHUNK, "the bound on the number of chunks assumes it");
+__device__ __forceinline__ uint32_t mp_class(uint32_t cnt) { return NFM_LANE_MAX - cnt; }   // longest first
 __global__ void __launch_bounds__(256) k_mp_hist(int ncell, const uint32_t *__restrict__ offsets, uint32_t *__restrict__ hist) {
     __shared__ uint32_t h[NFM_NCLASS];
     for (int i = threadIdx.x; i < NFM_NCLASS; i += blockDim.x) h[i] = 0u;
     __syncthreads();
-    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += gridDim.x * blockDim.x) atomicAdd(&h[mp_class(offsets[c + 1] - offsets[c])], 1u);
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += gridDim.x * blockDim.x) {
+        const uint32_t n = offsets[c + 1] - offsets[c];
+        if (n <= NFM_LANE_MAX) atomicAdd(&h[mp_class(n)], 1u);
+        else {
+            atomicAdd(&h[mp_class(NFM_CHUNK)], n / NFM_CHUNK);
+            if (n % NFM_CHUNK) atomicAdd(&h[mp_class(n % NFM_CHUNK)], 1u);
+        }
+    }
     __syncthreads();
     for (int i = threadIdx.x; i < NFM_NCLASS; i += blockDim.x) if (h[i]) atomicAdd(&hist[i], h[i]);
 }
@@ -168,18 +184,21 @@ __global__ void __launch_bounds__(256) k_mp_scan(uint32_t *hist) {      // one b
     for (int k = 0; k < PER; ++k) { const int i = threadIdx.x * PER + k; v[k] = i < NFM_NCLASS ? hist[i] : 0u; s += v[k]; }
     part[threadIdx.x] = s;
     __syncthreads();
-    if (threadIdx.x == 0) { uint32_t t = 0; for (int i = 0; i < 256; ++i) { const uint32_t x = part[i]; part[i] = t; t += x; } }
+    if (threadIdx.x == 0) { uint32_t t = 0; for (int i = 0; i < 256; ++i) { const uint32_t x = part[i]; part[i] = t; t += x; } hist[NFM_NCLASS] = t; }
     __syncthreads();
     uint32_t e = part[threadIdx.x];
 #pragma unroll
     for (int k = 0; k < PER; ++k) {
         const int i = threadIdx.x * PER + k;
-        if (i < NFM_NCLASS) { hist[i] = e; if (i == NFM_NCLASS - 1) hist[NFM_NCLASS] = e; }
+        if (i < NFM_NCLASS) hist[i] = e;
         e += v[k];
     }
 }
+struct MpItems { uint32_t *cell, *chunk, *pidx; };     // item w: particles [chunk * NFM_CHUNK, ...) of `cell`; pidx = its partial (0xffffffff: straight to M)
+struct MpDense { uint32_t cell, first, nchunk; };      // a dense cell: its partials are first .. first + nchunk - 1
 #define NFM_FILL_ITEMS 8
-__global__ void __launch_bounds__(256) k_mp_fill(int ncell, const uint32_t *__restrict__ offsets, uint32_t *__restrict__ hist, uint32_t *__restrict__ order) {
+__global__ void __launch_bounds__(256) k_mp_fill(int ncell, const uint32_t *__restrict__ offsets, uint32_t *__restrict__ hist, MpItems I,
+                                                 MpDense *__restrict__ dense) {
     __shared__ uint32_t h[NFM_NCLASS];
     for (int i = threadIdx.x; i < NFM_NCLASS; i += blockDim.x) h[i] = 0u;
     __syncthreads();
@@ -188,7 +207,22 @@ __global__ void __launch_bounds__(256) k_mp_fill(int ncell, const uint32_t *__re
 #pragma unroll
     for (int k = 0; k < NFM_FILL_ITEMS; ++k) {
         const int c = c0 + k * 256;
-        if (c < ncell) { cls[k] = mp_class(offsets[c + 1] - offsets[c]); rank[k] = atomicAdd(&h[cls[k]], 1u); }
+        cls[k] = 0xffffffffu;
+        if (c < ncell) {
+            const uint32_t n = offsets[c + 1] - offsets[c];
+            if (n <= NFM_LANE_MAX) { cls[k] = mp_class(n); rank[k] = atomicAdd(&h[cls[k]], 1u); }
+            else {                                            // a dense cell (rare): its chunks take their places one by one
+                const uint32_t nch = (n + NFM_CHUNK - 1) / NFM_CHUNK;
+                const uint32_t first = atomicAdd(&hist[NFM_CTR_CHUNK], nch);
+                MpDense d; d.cell = (uint32_t)c; d.first = first; d.nchunk = nch;
+                dense[atomicAdd(&hist[NFM_CTR_DENSE], 1u)] = d;
+                for (uint32_t ch = 0; ch < nch; ++ch) {
+                    const uint32_t cnt = (ch + 1u) * NFM_CHUNK <= n ? NFM_CHUNK : n - ch * NFM_CHUNK;
+                    const uint32_t w = atomicAdd(&hist[mp_class(cnt)], 1u);
+                    I.cell[w] = (uint32_t)c; I.chunk[w] = ch; I.pidx[w] = first + ch;
+                }
+            }
+        }
     }
     __syncthreads();
     for (int i = threadIdx.x; i < NFM_NCLASS; i += blockDim.x) if (h[i]) h[i] = atomicAdd(&hist[i], h[i]);      // the block's range in class i
@@ -196,19 +230,36 @@ __global__ void __launch_bounds__(256) k_mp_fill(int ncell, const uint32_t *__re
 #pragma unroll
     for (int k = 0; k < NFM_FILL_ITEMS; ++k) {
         const int c = c0 + k * 256;
-        if (c < ncell) order[h[cls[k]] + rank[k]] = (uint32_t)c;
+        if (cls[k] != 0xffffffffu) { const uint32_t w = h[cls[k]] + rank[k]; I.cell[w] = (uint32_t)c; I.chunk[w] = 0u; I.pidx[w] = 0xffffffffu; }
     }
 }
 
 template <int P>
-__global__ void __launch_bounds__(128, 2) k_multipoles_cells(const MultipoleArgs A) {
+__global__ void __launch_bounds__(128, 2) k_multipoles_cells(const MultipoleArgs A, const MpItems I, const uint32_t *__restrict__ nitems,
+                                                             double *__restrict__ partial) {
     const uint32_t w = blockIdx.x * blockDim.x + threadIdx.x;
-    if (w >= *A.nsmall) return;                           // the dense class: k_multipoles takes it
-    const int cell = (int)A.corder[w];
-    const uint32_t n = A.offsets[cell + 1] - A.offsets[cell];
-    const uint32_t p0 = A.poff[cell];
-    double *out = A.M + (size_t)cell * A.cml;
+    if (w >= *nitems) return;
+    const int cell = (int)I.cell[w];
+    const uint32_t j0 = I.chunk[w] * NFM_CHUNK, pidx = I.pidx[w];
+    const uint32_t ncell_p = A.offsets[cell + 1] - A.offsets[cell];
+    const uint32_t n = pidx == 0xffffffffu ? ncell_p : (j0 + NFM_CHUNK <= ncell_p ? NFM_CHUNK : ncell_p - j0);
+    const uint32_t p0 = A.poff[cell] + j0;                // chunks start on multiples of 4 slots
+    double *out = pidx == 0xffffffffu ? A.M + (size_t)cell * A.cml : partial + (size_t)pidx * A.cml;
     mp_all_slices<P, 0>(A, p0, n, out);
+}
+
+// M of a dense cell = its chunks' partials added in chunk order
+__global__ void __launch_bounds__(192) k_mp_reduce(const uint32_t *__restrict__ hist, const MpDense *__restrict__ dense, const double *__restrict__ partial,
+                                                   double *__restrict__ M, int cml) {
+    const uint32_t nd = hist[NFM_CTR_DENSE];
+    for (uint32_t d = blockIdx.x; d < nd; d += gridDim.x) {
+        const MpDense D = dense[d];
+        for (int e = threadIdx.x; e < cml; e += blockDim.x) {
+            double s = 0.0;
+            for (uint32_t ch = 0; ch < D.nchunk; ++ch) s += partial[(size_t)(D.first + ch) * cml + e];
+            M[(size_t)D.cell * cml + e] = s;
+        }
+    }
 }
 
 // PMAX = compile-time bound of the order (8: the paper's choice; NFM_MAX_ORDER: any order)
@@ -240,10 +291,7 @@ __global__ void __launch_bounds__(160) k_multipoles(const MultipoleArgs A) {
     int ncw = nc;
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) ncw = max(ncw, __shfl_xor_sync(0xffffffffu, ncw, d));
-    const int wstart = A.corder ? (int)*A.nsmall : 0;
-    const int nwork = A.ncell - wstart;
-    for (int w = blockIdx.x; w < nwork; w += gridDim.x) {
-        const int cell = A.corder ? (int)A.corder[wstart + w] : w;
+    for (int cell = blockIdx.x; cell < A.ncell; cell += gridDim.x) {
         const uint32_t p0 = A.offsets[cell], p1 = A.offsets[cell + 1];
         double acc[PMAX + 1];
 #pragma unroll
@@ -308,23 +356,28 @@ nf_status nf_run_multipoles(nf_ctx *ctx, const float *d_pos, int order, double *
     A.pos = d_pos; A.offsets = ctx->d_offsets; A.perm = ctx->d_perm_true; A.M = d_M;
     A.scale = ctx->prm.scale; A.cellsz = ctx->box / (double)ctx->cpd;
     A.ncell = (int)ctx->ncell; A.order = order; A.cml = (order + 3) * (order + 2) * (order + 1) / 6;
-    A.corder = nullptr; A.nsmall = nullptr; A.poff = ctx->d_poff; A.sorted = ctx->d_sorted; A.cap_pad = (uint32_t)ctx->capPad;
+    A.poff = ctx->d_poff; A.sorted = ctx->d_sorted; A.cap_pad = (uint32_t)ctx->capPad;
     const int64_t want = ctx->ncell;
     const int grid = (int)(want < (int64_t)ctx->sm_count * 2048 ? want : (int64_t)ctx->sm_count * 2048);
-    if (order == 8) {        // the paper's order: a lane per cell, then the cells too dense for that by the CTA-per-cell kernel
-        uint32_t *order = ctx->d_tmp_perm;                               // (d_tmp_perm is free once the binning is done)
+    if (order == 8) {        // the paper's order: a lane per work item (cell, or chunk of a dense cell), then the dense cells' partials are added
         uint32_t *hist = ctx->d_mp_hist;
-        NF_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, (NFM_NCLASS + 1) * sizeof(uint32_t), st));
+        MpItems I;                                                       // (d_tmp_perm, d_key and d_chunk_sorted are free once the binning is done)
+        const size_t icap = (size_t)ctx->capPad / 3;                     // >= ncell + N / NFM_CHUNK items
+        I.cell = ctx->d_tmp_perm; I.chunk = ctx->d_tmp_perm + icap; I.pidx = ctx->d_tmp_perm + 2 * icap;
+        MpDense *dense = reinterpret_cast<MpDense *>(ctx->d_key);        // <= N / NFM_LANE_MAX dense cells of 3 words
+        double *partial = reinterpret_cast<double *>(ctx->d_chunk_sorted);
+        NF_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, (NFM_NCLASS + 4) * sizeof(uint32_t), st));
         const int hgrid = (int)(want / 256 + 1 < (int64_t)ctx->sm_count * 8 ? want / 256 + 1 : (int64_t)ctx->sm_count * 8);
         k_mp_hist<<<hgrid, 256, 0, st>>>(A.ncell, A.offsets, hist); ctx->launches++;
         k_mp_scan<<<1, 256, 0, st>>>(hist); ctx->launches++;
-        k_mp_fill<<<(uint32_t)((want + 256 * NFM_FILL_ITEMS - 1) / (256 * NFM_FILL_ITEMS)), 256, 0, st>>>(A.ncell, A.offsets, hist, order); ctx->launches++;
-        A.corder = order; A.nsmall = hist + NFM_NCLASS;
-        k_multipoles_cells<8><<<(uint32_t)((want + 127) / 128), 128, 0, st>>>(A); ctx->launches++;
+        k_mp_fill<<<(uint32_t)((want + 256 * NFM_FILL_ITEMS - 1) / (256 * NFM_FILL_ITEMS)), 256, 0, st>>>(A.ncell, A.offsets, hist, I, dense); ctx->launches++;
+        const uint64_t items = (uint64_t)want + (uint64_t)ctx->lastN / NFM_CHUNK + 1;      // upper bound of the item count, known on the host
+        k_multipoles_cells<8><<<(uint32_t)((items + 127) / 128), 128, 0, st>>>(A, I, hist + NFM_NCLASS, partial); ctx->launches++;
+        k_mp_reduce<<<ctx->sm_count * 8, 192, 0, st>>>(hist, dense, partial, A.M, A.cml); ctx->launches++;
+        NF_CUDA_OK(ctx, cudaGetLastError());
+        return NF_OK;
     }
-    const int dgrid = order == 8 ? ctx->sm_count * 16 : grid;           // the dense cells only: their number is on the device
-    if (order == 8) k_multipoles<8><<<dgrid, nfm_threads(order), 0, st>>>(A);
-    else if (order < 8) k_multipoles<8><<<grid, nfm_threads(order), 0, st>>>(A);
+    if (order < 8) k_multipoles<8><<<grid, nfm_threads(order), 0, st>>>(A);
     else k_multipoles<NFM_MAX_ORDER><<<grid, nfm_threads(order), 0, st>>>(A);
     ctx->launches++;
     NF_CUDA_OK(ctx, cudaGetLastError());

@@ -3,8 +3,12 @@
 Every element is a double sum of monomials in the same particle order on both sides; the kernel
 forms x^a y^b z^c as (x^a y^b) z^c with the last product fused into the add (the FMA form of
 PAPER.md:199), the oracle by the pseudo-code's running products, so terms differ by a few ulp
-and sums by the rounding of n additions: bar |dM| <= 1e-13 * sum_q |x^a y^b z^c| per element
-(counts, a = b = c = 0, are exact)."""
+and sums by the rounding of n additions.  Bar per element, with S = sum_q |x^a y^b z^c| and n the cell's
+occupancy: |dM| <= (1e-13 + 2.3e-16 n) S -- the second term is the forward error bound (n - 1) u S of a
+recursive double sum (u = 2^-53), which the ORACLE's sequential sum of a long cell exhausts first: in the
+8404-particle cell of the clustered case the oracle is 2.7e-11 and the kernel (512-particle chunks, then
+the partials) 1.6e-12 from the exactly rounded sum.  So the dense cells are ALSO held against math.fsum
+of the same double offsets, at 1e-13 S without the n term (counts, a = b = c = 0, are exact)."""
 import numpy as np
 import pytest
 
@@ -56,7 +60,20 @@ def test_multipoles_match_the_oracle(torch_cuda, NF, oracle_mod, label, cfg, ord
     assert got.shape == ref.shape == (cfg.cpd ** 3, len(idx))
     assert np.array_equal(got[:, 0], ref[:, 0])                              # occupancy: exact
     scale = _abs_moments(pos, cfg.cpd, order, idx)
-    assert np.all(np.abs(got - ref) <= 1e-13 * scale + 1e-300), label
+    n = ref[:, :1]
+    assert np.all(np.abs(got - ref) <= (1e-13 + 2.3e-16 * n) * scale + 1e-300), label
+    # the cells of more than 512 particles (chunked on the GPU) against the exactly rounded sums
+    import math
+    t = pos.astype(np.float64) * cfg.cpd
+    c = np.floor(t).astype(np.int64) % cfg.cpd
+    key = (c[:, 0] * cfg.cpd + c[:, 1]) * cfg.cpd + c[:, 2]
+    off = (t - np.floor(t) - 0.5) / cfg.cpd
+    for cell in np.flatnonzero(ref[:, 0] > 512)[:6]:
+        o = off[key == cell]
+        for col in sorted({1, len(idx) // 3, len(idx) - 1} & set(range(len(idx)))):
+            a, b, k = idx[col]
+            exact = math.fsum((o[:, 0] ** a * o[:, 1] ** b * o[:, 2] ** k).tolist())
+            assert abs(got[cell, col] - exact) <= 1e-13 * scale[cell, col] + 1e-300, (label, int(cell), (a, b, k))
 
 
 def test_multipoles_edge_cases(torch_cuda, NF, oracle_mod):
@@ -74,6 +91,36 @@ def test_multipoles_edge_cases(torch_cuda, NF, oracle_mod):
     key = (3 * 7 + 3) * 7 + 3
     assert got[key, 0] == 777 and np.count_nonzero(np.delete(got, key, axis=0)) == 0
     assert np.allclose(got, ref, rtol=1e-12, atol=1e-30)
+
+
+def test_multipoles_chunk_boundaries(torch_cuda, NF, oracle_mod):
+    """cells on either side of the lane limit (1024) and of the 512-particle chunk size, shuffled input"""
+    import math
+    rng = np.random.default_rng(12)
+    cpd = 5
+    sizes = {(0, 0, 0): 1024, (1, 1, 1): 1025, (2, 2, 2): 1536, (3, 3, 3): 2049, (4, 4, 4): 511, (0, 4, 2): 513, (2, 0, 3): 5000}
+    pos = np.concatenate([((np.array(c) + rng.random((n, 3))) / cpd) for c, n in sizes.items()])
+    pos = pos[rng.permutation(len(pos))].astype(np.float32)
+    pos[pos >= 1.0] = 0.0
+    with NF(cpd, 2, 1e-3, 1.0) as nf:
+        M = nf.multipoles(torch_cuda.from_numpy(pos).cuda(), 8)
+        nf.sync()
+        got = M.cpu().numpy()
+    ref = oracle_mod.multipoles(pos, cpd, 8)
+    idx = oracle_mod.multipole_index(8)
+    scale = _abs_moments(pos, cpd, 8, idx)
+    assert np.array_equal(got[:, 0], ref[:, 0])
+    assert np.all(np.abs(got - ref) <= (1e-13 + 2.3e-16 * ref[:, :1]) * scale + 1e-300)
+    t = pos.astype(np.float64) * cpd
+    c = np.floor(t).astype(np.int64) % cpd
+    key = (c[:, 0] * cpd + c[:, 1]) * cpd + c[:, 2]
+    off = (t - np.floor(t) - 0.5) / cpd
+    for cell in np.flatnonzero(ref[:, 0] > 0):
+        o = off[key == cell]
+        for col in (1, 9, 45, 100, 164):
+            a, b, k = idx[col]
+            exact = math.fsum((o[:, 0] ** a * o[:, 1] ** b * o[:, 2] ** k).tolist())
+            assert abs(got[cell, col] - exact) <= 1e-13 * scale[cell, col] + 1e-300, (int(cell), (a, b, k))
 
 
 def test_multipoles_full_size_config4_properties(torch_cuda, NF):
