@@ -364,6 +364,9 @@ def measure(k: int, args, rank: int, world: int, local_rank: int, dist, barrier,
         "measured_mufu_rsq_lane_ops_per_s": peaks_live["mufu_rsq_lane_ops_per_s"],
         "measured_dfma_lane_ops_per_s": peaks_live["dfma_lane_ops_per_s"],
         "mufu_frac": pairs / (k_ms * 1e-3) / peaks_live["mufu_rsq_lane_ops_per_s"]}
+    if k == 4:          # the microbenchmarks behind DESIGN.md section 6 (register operands of packed instructions, trip-loop replica)
+        from paper_2110_11392_b200.opbench import operand_probe
+        out["roofline"]["operand_probe"] = operand_probe(sm_max)
     out["stage_ms"] = {kk: statistics.mean(st[kk] for st in stage_acc) for kk in stage_acc[0]}
     if args.neighbours:
         out["neighbour_steps"] = _neighbour_steps(nf, d_pos, d_acc, cfg, peaks_live)

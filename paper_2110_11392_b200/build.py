@@ -6,6 +6,8 @@
 * ``libnf_pipeprobe.so``   -- a bench-only helper (``csrc/probe/nf_pipeprobe.cu``): FP32 / FP64 / MUFU
   pipe-rate microbenchmarks that give ``bench.py`` its live roofline denominators.  Not part of the
   product ABI.
+* ``libnf_opbench.so``     -- a bench-only helper (``microbench/nf_opbench.cu``): the register-operand and
+  trip-loop-replica microbenchmarks behind DESIGN.md section 6 (``python -m paper_2110_11392_b200.opbench``).
 
 nvcc cross-compiles without a GPU.  The .so files are git-ignored but travel with the repo snapshot.
 Translation units are compiled in parallel and linked once.
@@ -22,6 +24,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnearfield_b200.so")
 PROBE_LIB = os.path.join(HERE, "libnf_pipeprobe.so")
+OPBENCH_LIB = os.path.join(HERE, "libnf_opbench.so")
+OPBENCH_SRC = os.path.join(HERE, "microbench", "nf_opbench.cu")
 SOURCES = ["nf_api.cu", "nf_binner.cu", "nf_rebin.cu", "nf_interact.cu", "nf_f64.cu", "nf_multipoles.cu", "nf_taylor.cu", "nf_step.cu",
            "nf_slabs.cu"]
 PROBE_SOURCES = [os.path.join("probe", "nf_pipeprobe.cu")]
@@ -54,6 +58,30 @@ def _stale(lib: str) -> bool:
             return not os.path.exists(lib) or f.read().strip() != _source_hash()
     except OSError:
         return True
+
+
+def _opbench_stale() -> bool:
+    import hashlib
+    with open(OPBENCH_SRC, "rb") as f:
+        h = hashlib.sha1(f.read()).hexdigest()
+    try:
+        with open(OPBENCH_LIB + ".srchash") as f:
+            return not os.path.exists(OPBENCH_LIB) or f.read().strip() != h
+    except OSError:
+        return True
+
+
+def _compile_opbench(verbose: bool) -> None:
+    """one translation unit of its own (kept out of csrc/: the product library's state tag does not depend on it)"""
+    import hashlib
+    nvcc = os.environ.get("NVCC", "nvcc")
+    cmd = [nvcc, *NVCC_FLAGS, "-shared", "-o", OPBENCH_LIB + ".tmp", OPBENCH_SRC]
+    if verbose:
+        cmd.insert(1, "-Xptxas=-v")
+    subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
+    os.replace(OPBENCH_LIB + ".tmp", OPBENCH_LIB)
+    with open(OPBENCH_SRC, "rb") as f, open(OPBENCH_LIB + ".srchash", "w") as g:
+        g.write(hashlib.sha1(f.read()).hexdigest() + "\n")
 
 
 def _compile(sources: list[str], lib: str, verbose: bool) -> None:
@@ -90,6 +118,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         _compile(SOURCES, LIB, verbose)
     if force or _stale(PROBE_LIB):
         _compile(PROBE_SOURCES, PROBE_LIB, verbose)
+    if force or _opbench_stale():
+        _compile_opbench(verbose)
     return LIB
 
 
@@ -120,7 +150,7 @@ def ensure_built() -> str:
     """Make sure the in-tree libraries exist and are not older than their sources (a fresh checkout
     has none: they are not tracked).  A build step, not a fallback: without nvcc a stale or missing
     library raises instead of being loaded silently."""
-    if _stale(LIB) or _stale(PROBE_LIB):
+    if _stale(LIB) or _stale(PROBE_LIB) or _opbench_stale():
         build_library()
     return LIB
 

@@ -19,6 +19,7 @@ import numpy as np, torch
 import paper_2110_11392_b200.binding as B
 from paper_2110_11392_b200 import workloads as W
 import oracle
+torch.manual_seed(0)
 assert B.bounds_checked(), "not the NF_DEBUG_BOUNDS build"
 assert B.lib_path().startswith(r"%(copy)s"), B.lib_path()
 

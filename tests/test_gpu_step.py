@@ -131,6 +131,7 @@ def test_bin_once_reuse_everywhere(torch_cuda, NF, oracle_mod):
         M_pin = nf.multipoles(d_pos, 4)
         assert nf.launch_count() - n2 == 1
         f_pin = nf.accel_f64(d_pos)
+        torch.manual_seed(1)
         T = torch.randn_like(M_pin)
         y_pin = nf.taylor_accel(d_pos, T, 4).clone()
         t_pin = nf.timestep_ratio(d_pos, d_vel, a_plain)
@@ -224,7 +225,8 @@ def test_rebin_without_a_binning_and_with_another_count(torch_cuda, NF, oracle_m
         g = nf.debug_cells()
         assert np.array_equal(g["offsets"].astype(np.int64), o2) and np.array_equal(g["perm"].astype(np.int64), r2)
         # everything into one cell, then spread out again
-        one = ((3 + torch.rand((cfg.N // 2, 3), device="cuda")) / cfg.cpd).contiguous()
+        gen = torch.Generator(device="cuda").manual_seed(5)        # seeded, and away from the cell's upper face: (3 + u)/cpd must not round into cell 4
+        one = ((3 + 0.999 * torch.rand((cfg.N // 2, 3), device="cuda", generator=gen)) / cfg.cpd).contiguous()
         nf.rebin(one)
         g = nf.debug_cells()
         assert int(g["offsets"][-1]) == cfg.N // 2 and int(np.diff(g["offsets"].astype(np.int64)).max()) == cfg.N // 2
