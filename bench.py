@@ -406,6 +406,7 @@ def _neighbour_steps(nf, d_pos, d_acc, cfg, peaks_live, order: int = 8) -> dict:
     del M
     vel = torch.zeros_like(d_pos)
     res["kick_drift_ms"] = timed(lambda: nf.kick_drift(d_pos, vel, d_acc, 0.0, 0.0))
+    res["timestep_ratio_ms"] = timed(lambda: nf.timestep_ratio(d_pos, vel, d_acc))          # Eq. 1's per-cell reduction (on the pinned binning; syncs)
     # nf_rebin after a drift of 0.05 cell rms per component (a few per cent of the particles change cell: PAPER.md:356
     # "most particles stay in their cell") against the full sort above; the drift itself is not timed
     vel = torch.randn_like(d_pos) * (0.05 * cfg.box / cfg.cpd)
