@@ -233,10 +233,13 @@ def _box_filter(n: np.ndarray, R: int) -> np.ndarray:
     return f
 
 
+W_BASE_CPD = {1: 7, 2: 35, 3: 63, 4: 135, 5: 45}
+
+
 def _workload(k: int, cfg, world: int, parallel: str) -> dict:
     par = "single GPU" if world == 1 else (f"x-slab decomposition over {world} GPUs, R-slab halo exchange per step" if parallel == "slabs"
                                            else f"replicas x{world}")
-    return {"workload": f"BASELINE.json configs[{k - 1}]: {cfg.name} CPD={cfg.cpd} R={cfg.R} N={cfg.N} "
+    return {"workload": f"{'BASELINE.json' if cfg.cpd == W_BASE_CPD.get(k) else 'size study, recipe of BASELINE.json'} configs[{k - 1}]: {cfg.name} CPD={cfg.cpd} R={cfg.R} N={cfg.N} "
                         f"eps_p={cfg.eps_p:.6g} box=1 kind={cfg.kind} seed={'0' if parallel == 'slabs' or world == 1 else 'rank'}",
             "cpd": cfg.cpd, "R": cfg.R, "N": cfg.N, "parallelism": par,
             "l2_policy": "inputs (1.9 GB positions, ~9 GB scratch) exceed the 126 MB L2; no flush needed"
@@ -263,7 +266,7 @@ def measure(k: int, args, rank: int, world: int, local_rank: int, dist, barrier,
     from paper_2110_11392_b200 import workloads as W
     from paper_2110_11392_b200.binding import NearField
     from paper_2110_11392_b200.pipeprobe import probe_pipes
-    base = W.CONFIGS[k]
+    base = W.CONFIGS[k] if not getattr(args, "scale_cpd", 0) else W.scaled(W.CONFIGS[k], args.scale_cpd)
     cfg = W.Config(base.name, base.cpd, base.R, base.N, base.kind, base.eps_p, base.box, seed=seed, n_spheres=base.n_spheres)
     pos = W.make_positions(cfg)
     nf = NearField(cfg.cpd, cfg.R, cfg.eps_p, cfg.box)
@@ -530,6 +533,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="all", help="'all' (default): BASELINE.json config 4 (CPD 135, N 157M) as the headline of the line plus "
                                                     "configs 1, 2, 3, 5 under per_config; or one config number 1..5")
+    ap.add_argument("--scale-cpd", type=int, default=0, help="with --config K: run config K's RECIPE (particles per cell, distribution, "
+                    "softening rule) on a grid of this many cells per dimension instead of its own -- a size study, not a BASELINE.json workload "
+                    "(e.g. --config 2 --scale-cpd 100: 40 per cell, 40 M particles)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target pair-loop time of the oracle for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -547,7 +553,9 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    want_all = args.config == "all"
+    want_all = args.config == "all" and not args.scale_cpd
+    if args.scale_cpd and args.config == "all":
+        raise SystemExit("bench.py: --scale-cpd needs --config K")
     k_main = 4 if want_all else int(args.config)
     slabs_mode = (world > 1 and args.parallel != "replicas") or args.parallel == "slabs"
 
