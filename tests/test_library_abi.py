@@ -82,3 +82,18 @@ def test_product_does_not_import_oracle():
             with open(os.path.join(ROOT, "oracle", fn)) as f:
                 t = f.read()
             assert "import paper_2110_11392_b200" not in t and "from paper_2110_11392_b200" not in t and "nearfield.h" not in t, fn
+
+
+def test_bench_only_helper_libraries_are_built_and_separate():
+    """libnf_pipeprobe.so / libnf_opbench.so (bench-only microbenchmarks) are built by build() beside the product
+    library, export their one entry point each, and export none of the product's nf_* symbols (and vice versa)."""
+    import ctypes
+    from paper_2110_11392_b200 import build
+    build.ensure_built()
+    probe = ctypes.CDLL(build.PROBE_LIB)
+    opb = ctypes.CDLL(build.OPBENCH_LIB)
+    prod = ctypes.CDLL(build.LIB)
+    assert hasattr(probe, "nfp_probe_pipes") and hasattr(opb, "nfo_opbench")
+    for helper in (probe, opb):
+        assert not hasattr(helper, "nf_accel") and not hasattr(helper, "nf_create")
+    assert not hasattr(prod, "nfp_probe_pipes") and not hasattr(prod, "nfo_opbench")
