@@ -176,6 +176,49 @@ nf_status nf_select_slabs(nf_ctx *ctx, const float *d_pos, int64_t N, int x0, in
                           void *cuda_stream);
 
 /*
+ * nf_cell_offsets_noalloc -- step A2 without a context and without any allocation: the exclusive scan
+ * of a cell histogram into the per-cell offsets of the grid order (each cell is an
+ * offset and a count into the grid-ordered arrays),
+ *     d_offsets[c] = sum of d_counts[c'] over c' < c,   d_offsets[ncell] = the total.
+ *
+ * For callers that cannot let a library call cudaMalloc.  Everything else in this header works on an
+ * nf_ctx whose scratch comes from cudaMalloc, at nf_create and again when a larger N arrives.  That
+ * does not suit (a) a code that gave the whole device to its own memory pool at start-up, as a
+ * simulation sized to fill the GPU does -- a later cudaMalloc can just fail; or (b) a time-step loop
+ * that keeps copies and kernels in flight on several streams -- cudaMalloc and cudaFree wait for the
+ * whole device and break that overlap.  This call touches only the caller's two buffers and a fixed
+ * array of tile partial sums that is part of the library's device image.  It calls no cudaMalloc,
+ * cudaFree or allocating library routine, and needs no context.
+ *
+ *   d_counts   [in]  device, ncell int32, non-negative, total below 2^32 (e.g. nf_cell_histogram's
+ *                    output, key = (cx*cpd+cy)*cpd+cz).  May be NULL when ncell == 0.
+ *   d_offsets  [out] device, ncell + 1 uint32.  Must not overlap d_counts.  Caller-owned, like d_counts.
+ *   cuda_stream      cudaStream_t as void*; both launches are enqueued there, no synchronisation.
+ *
+ * Limits and rules
+ *   - ncell <= NF_NOALLOC_MAX_CELLS (8 388 608 = 4096 tiles of 2048 cells, i.e. cpd <= 203; the
+ *     157 M-particle configuration has 135^3 = 2 460 375).  A larger ncell is refused with NF_EINVAL
+ *     and a message that names the limit; nothing is launched.  Use a context (nf_bin) there.
+ *   - Cost of the fixed array: 16 KB of device memory on every GPU that loads this library, from the
+ *     load until the process exits, whether or not this call is ever made.
+ *   - The device that holds the buffers (and owns the stream) must be the CURRENT device.  The first
+ *     call on each device looks up the array's device address (cudaGetSymbolAddress) and remembers
+ *     it; make that first call before any stream capture begins on that device.
+ *   - All calls on a device share the one array.  It keeps whatever the previous call left; nothing in
+ *     it has to start at zero, because each call writes every word it later reads.  Two calls whose
+ *     kernels can overlap on the GPU (different streams with no ordering between them) race on the
+ *     array and give wrong offsets: order them (same stream, or an event).  Host threads may call
+ *     concurrently (the set-up is locked); the ordering of the GPU work is still the caller's job.
+ *   - Result equals the context path's offsets (nf_debug_cells after nf_bin) bit for bit.
+ * Errors: NF_EINVAL -- ncell < 0 or beyond the limit, d_offsets NULL, d_counts NULL with ncell > 0;
+ * NF_ECUDA -- no current device, the address look-up or a launch failed.  The text is returned by
+ * nf_cell_offsets_noalloc_error (static storage, valid until the next failing call).
+ */
+#define NF_NOALLOC_MAX_CELLS 8388608
+nf_status nf_cell_offsets_noalloc(const int32_t *d_counts, int64_t ncell, uint32_t *d_offsets, void *cuda_stream);
+const char *nf_cell_offsets_noalloc_error(void);
+
+/*
  * nf_accel4 -- nf_accel with the accelerations "promoted to 4-vectors":
  *   d_acc4 [out] device, N*4 floats (ax, ay, az, w) in INPUT order, where
  *       w_i = sum over the sources j != i of the same (2R+1)^3 cells with r_ij < b of (b^2 - r_ij^2),

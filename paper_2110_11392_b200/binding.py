@@ -23,7 +23,8 @@ SYMBOLS = ["nf_create", "nf_destroy", "nf_set_gm", "nf_accel", "nf_accel_host", 
            "nf_last_error", "nf_set_option", "nf_stage_ms", "nf_debug_cells", "nf_debug_neighbors",
            "nf_interaction_count", "nf_debug_read", "nf_launch_count", "nf_close_radius",
            "nf_set_softening", "nf_set_density_radius", "nf_accel4", "nf_set_sink_slabs", "nf_accel_f64", "nf_multipoles", "nf_kick_drift", "nf_timestep_ratio", "nf_taylor_accel",
-           "nf_debug_delivered_pairs", "nf_bounds_checked", "nf_bin", "nf_rebin", "nf_unbin", "nf_cell_histogram", "nf_slab_pairs", "nf_select_slabs"]
+           "nf_debug_delivered_pairs", "nf_bounds_checked", "nf_bin", "nf_rebin", "nf_unbin", "nf_cell_histogram", "nf_slab_pairs", "nf_select_slabs",
+           "nf_cell_offsets_noalloc", "nf_cell_offsets_noalloc_error"]
 
 
 class NearFieldError(RuntimeError):
@@ -109,6 +110,10 @@ def load_library() -> ctypes.CDLL:
     L.nf_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     L.nf_debug_read.restype = i32
     L.nf_debug_read.argtypes = [vp, vp, vp, ctypes.c_uint64]
+    L.nf_cell_offsets_noalloc.restype = i32
+    L.nf_cell_offsets_noalloc.argtypes = [vp, i64, vp, vp]
+    L.nf_cell_offsets_noalloc_error.restype = ctypes.c_char_p
+    L.nf_cell_offsets_noalloc_error.argtypes = []
     return L
 
 
@@ -118,6 +123,32 @@ _L = load_library()
 def bounds_checked() -> bool:
     """nf_bounds_checked: is the loaded library the -DNF_DEBUG_BOUNDS build?"""
     return bool(_L.nf_bounds_checked())
+
+
+NF_NOALLOC_MAX_CELLS = 8388608
+
+
+def cell_offsets_noalloc(counts, offsets=None, stream=None):
+    """nf_cell_offsets_noalloc: exclusive scan of a cell histogram (CUDA int32 [ncell]) into ``offsets`` (CUDA int32 /
+    uint32 storage, [ncell + 1]) with no context and no device allocation inside the library -- for callers that
+    cannot let a library call cudaMalloc (a code whose own pool holds the whole GPU; a loop whose overlapping streams
+    a cudaMalloc would stall).  Pass ``offsets`` yourself to keep the call free of any allocation: when it is None
+    this wrapper -- not the library -- makes the tensor with torch.  The tensors' device must be the current device.
+    At most NF_NOALLOC_MAX_CELLS cells; calls that may overlap on the GPU race on the shared scratch (see nearfield.h)."""
+    import torch
+    if not (counts.is_cuda and counts.dtype == torch.int32 and counts.is_contiguous() and counts.dim() == 1):
+        raise ValueError("counts must be a contiguous 1-D CUDA int32 tensor")
+    n = counts.numel()
+    if offsets is None:
+        offsets = torch.empty(n + 1, dtype=torch.int32, device=counts.device)
+    elif not (offsets.is_cuda and offsets.dtype == torch.int32 and offsets.is_contiguous() and offsets.numel() == n + 1
+              and offsets.device == counts.device):
+        raise ValueError("offsets must be a contiguous CUDA int32 tensor of ncell + 1 entries on counts' device")
+    st = torch.cuda.current_stream(counts.device) if stream is None else stream
+    rc = _L.nf_cell_offsets_noalloc(counts.data_ptr() if n else None, n, offsets.data_ptr(), ctypes.c_void_p(st.cuda_stream))
+    if rc != NF_OK:
+        raise NearFieldError(rc, _L.nf_cell_offsets_noalloc_error().decode())
+    return offsets
 
 
 class NearField:

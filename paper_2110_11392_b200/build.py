@@ -27,7 +27,7 @@ PROBE_LIB = os.path.join(HERE, "libnf_pipeprobe.so")
 OPBENCH_LIB = os.path.join(HERE, "libnf_opbench.so")
 OPBENCH_SRC = os.path.join(HERE, "microbench", "nf_opbench.cu")
 SOURCES = ["nf_api.cu", "nf_binner.cu", "nf_rebin.cu", "nf_interact.cu", "nf_f64.cu", "nf_multipoles.cu", "nf_taylor.cu", "nf_step.cu",
-           "nf_slabs.cu"]
+           "nf_slabs.cu", "nf_noalloc.cu"]
 PROBE_SOURCES = [os.path.join("probe", "nf_pipeprobe.cu")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-Wno-format-truncation"]
