@@ -3,11 +3,9 @@
 ``python -m paper_2110_11392_b200.build`` (or ``__graft_entry__.build()``) makes
 
 * ``libnearfield_b200.so`` -- the product: the C ABI of ``include/nearfield.h``;
-* ``libnf_pipeprobe.so``   -- a bench-only helper (``csrc/probe/nf_pipeprobe.cu``): FP32 / FP64 / MUFU
-  pipe-rate microbenchmarks that give ``bench.py`` its live roofline denominators.  Not part of the
-  product ABI.
-* ``libnf_opbench.so``     -- a bench-only helper (``microbench/nf_opbench.cu``): the register-operand and
-  trip-loop-replica microbenchmarks behind DESIGN.md section 6 (``python -m paper_2110_11392_b200.opbench``).
+* ``libnf_pipeprobe.so``   -- a bench-only helper (``probe/nf_pipeprobe.cu``, outside ``csrc/``: the product
+  library's state tag does not depend on it): FP32 / FP64 / MUFU pipe-rate microbenchmarks that give
+  ``bench.py`` its live roofline denominators.  Not part of the product ABI.
 
 nvcc cross-compiles without a GPU.  The .so files are git-ignored but travel with the repo snapshot.
 Translation units are compiled in parallel and linked once.
@@ -24,11 +22,9 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnearfield_b200.so")
 PROBE_LIB = os.path.join(HERE, "libnf_pipeprobe.so")
-OPBENCH_LIB = os.path.join(HERE, "libnf_opbench.so")
-OPBENCH_SRC = os.path.join(HERE, "microbench", "nf_opbench.cu")
+PROBE_SRC = os.path.join(HERE, "probe", "nf_pipeprobe.cu")
 SOURCES = ["nf_api.cu", "nf_binner.cu", "nf_rebin.cu", "nf_interact.cu", "nf_f64.cu", "nf_multipoles.cu", "nf_taylor.cu", "nf_step.cu",
            "nf_slabs.cu", "nf_noalloc.cu"]
-PROBE_SOURCES = [os.path.join("probe", "nf_pipeprobe.cu")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-Wno-format-truncation"]
 
@@ -60,44 +56,60 @@ def _stale(lib: str) -> bool:
         return True
 
 
-def _opbench_stale() -> bool:
+def _probe_stale() -> bool:
     import hashlib
-    with open(OPBENCH_SRC, "rb") as f:
+    with open(PROBE_SRC, "rb") as f:
         h = hashlib.sha1(f.read()).hexdigest()
     try:
-        with open(OPBENCH_LIB + ".srchash") as f:
-            return not os.path.exists(OPBENCH_LIB) or f.read().strip() != h
+        with open(PROBE_LIB + ".srchash") as f:
+            return not os.path.exists(PROBE_LIB) or f.read().strip() != h
     except OSError:
         return True
 
 
-def _compile_opbench(verbose: bool) -> None:
-    """one translation unit of its own (kept out of csrc/: the product library's state tag does not depend on it)"""
+def _compile_probe(verbose: bool) -> None:
+    """one translation unit of its own, kept out of csrc/"""
     import hashlib
     nvcc = os.environ.get("NVCC", "nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, "-shared", "-o", OPBENCH_LIB + ".tmp", OPBENCH_SRC]
+    cmd = [nvcc, *NVCC_FLAGS, "-shared", "-o", PROBE_LIB + ".tmp", PROBE_SRC]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
-    os.replace(OPBENCH_LIB + ".tmp", OPBENCH_LIB)
-    with open(OPBENCH_SRC, "rb") as f, open(OPBENCH_LIB + ".srchash", "w") as g:
+    os.replace(PROBE_LIB + ".tmp", PROBE_LIB)
+    with open(PROBE_SRC, "rb") as f, open(PROBE_LIB + ".srchash", "w") as g:
         g.write(hashlib.sha1(f.read()).hexdigest() + "\n")
 
 
 def _compile(sources: list[str], lib: str, verbose: bool) -> None:
+    import hashlib
     nvcc = os.environ.get("NVCC", "nvcc")
     os.makedirs(OBJ, exist_ok=True)
-    headers = [d for d in _deps() if d.endswith((".cuh", ".h"))]
-    newest_header = max(os.path.getmtime(h) for h in headers)
+    hh = hashlib.sha1(" ".join(NVCC_FLAGS).encode())
+    for h in sorted(d for d in _deps() if d.endswith((".cuh", ".h"))):
+        with open(h, "rb") as f:
+            hh.update(f.read())
 
     def one(src: str) -> str:
+        # an object is reused only if it was compiled from exactly this source, these headers and these flags:
+        # the key is a content hash kept beside the .o (mtimes do not survive a copy of the tree)
         path = os.path.join(CSRC, src)
         obj = os.path.join(OBJ, src.replace(os.sep, "_") + ".o")
-        if not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(path), newest_header):
+        k = hh.copy()
+        with open(path, "rb") as f:
+            k.update(f.read())
+        key = k.hexdigest()
+        try:
+            with open(obj + ".srchash") as f:
+                fresh = os.path.exists(obj) and f.read().strip() == key
+        except OSError:
+            fresh = False
+        if not fresh:
             cmd = [nvcc, *NVCC_FLAGS, "-c", "-o", obj, path]
             if verbose:
                 cmd.insert(1, "-Xptxas=-v")
             subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)
+            with open(obj + ".srchash", "w") as f:
+                f.write(key + "\n")
         return obj
 
     with ThreadPoolExecutor(max_workers=min(8, len(sources))) as ex:
@@ -116,10 +128,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
             os.remove(os.path.join(OBJ, f))
     if force or _stale(LIB):
         _compile(SOURCES, LIB, verbose)
-    if force or _stale(PROBE_LIB):
-        _compile(PROBE_SOURCES, PROBE_LIB, verbose)
-    if force or _opbench_stale():
-        _compile_opbench(verbose)
+    if force or _probe_stale():
+        _compile_probe(verbose)
     return LIB
 
 
@@ -150,7 +160,7 @@ def ensure_built() -> str:
     """Make sure the in-tree libraries exist and are not older than their sources (a fresh checkout
     has none: they are not tracked).  A build step, not a fallback: without nvcc a stale or missing
     library raises instead of being loaded silently."""
-    if _stale(LIB) or _stale(PROBE_LIB) or _opbench_stale():
+    if _stale(LIB) or _probe_stale():
         build_library()
     return LIB
 

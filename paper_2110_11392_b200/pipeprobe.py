@@ -1,6 +1,6 @@
 """Loader of ``libnf_pipeprobe.so`` -- a bench-only helper, not part of the product's C ABI.
 
-``probe_pipes()`` runs the pipe-rate microbenchmarks of ``csrc/probe/nf_pipeprobe.cu`` on the current
+``probe_pipes()`` runs the pipe-rate microbenchmarks of ``probe/nf_pipeprobe.cu`` on the current
 CUDA device; ``bench.py`` prints them as the live roofline denominators beside the derived peak.
 """
 from __future__ import annotations
