@@ -318,6 +318,15 @@ def measure(k: int, args, rank: int, world: int, local_rank: int, dist, barrier,
         h_pos = torch.from_numpy(pos).pin_memory()
         h_acc = torch.empty_like(h_pos).pin_memory()
         nf.accel_host_ptr(h_pos.data_ptr(), cfg.N, h_acc.data_ptr())          # warm-up (allocates staging)
+        # the link by itself: one plain pinned copy of the same bytes each way (outside the timed region), so that the
+        # reader can tell how much of e2e - value is PCIe and how much is the code
+        tmp = torch.empty_like(d_pos)
+        c0, c1, c2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        torch.cuda.synchronize()
+        c0.record(); tmp.copy_(h_pos, non_blocking=True); c1.record(); h_acc.copy_(tmp, non_blocking=True); c2.record()
+        torch.cuda.synchronize()
+        h2d_ms, d2h_ms = c0.elapsed_time(c1), c1.elapsed_time(c2)
+        del tmp
         barrier()
         t0 = time.perf_counter()
         n_e2e = max(1, min(args.steps, 3))
@@ -326,8 +335,14 @@ def measure(k: int, args, rank: int, world: int, local_rank: int, dist, barrier,
         barrier()
         e2e_ms_local = (time.perf_counter() - t0) * 1e3
         u2, t2 = aggregate_over_ranks(float(pairs) * n_e2e, e2e_ms_local, dist)
-        e2e = {"value": u2 / (t2 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": cfg.N * 12, "d2h_bytes_per_step": cfg.N * 12,
-               "steps": n_e2e, "ms_per_step": t2 / n_e2e, "api": "nf_accel_host (pinned host buffers; H2D chunks overlap the binning)"}
+        nbytes = cfg.N * 12
+        e2e = {"value": u2 / (t2 * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+               "steps": n_e2e, "ms_per_step": t2 / n_e2e, "api": "nf_accel_host (pinned host buffers; H2D chunks overlap the binning)",
+               "pcie_GBps": {"h2d": nbytes / (h2d_ms * 1e-3) / 1e9 if h2d_ms > 0 else None, "d2h": nbytes / (d2h_ms * 1e-3) / 1e9 if d2h_ms > 0 else None},
+               "plain_copy_ms": {"h2d": h2d_ms, "d2h": d2h_ms},
+               "ms_over_device_step": t2 / n_e2e - total_ms / args.steps,
+               "note": "the result is in input order and exists only after the kernel's fused un-permute, so the D2H copy follows the kernel "
+                       "serially (ms_over_device_step ~ plain_copy_ms.d2h + what of the H2D the binning cannot hide): the link, not the code"}
         del h_pos, h_acc
     out = {"value": value, "ms_per_step": total_ms / args.steps, "config": _workload(k, cfg, world, "replicas"),
            "sink_updates_per_s": cfg.N * world * args.steps / (total_ms * 1e-3), "pairs_per_step": pairs,
@@ -367,9 +382,6 @@ def measure(k: int, args, rank: int, world: int, local_rank: int, dist, barrier,
         "measured_mufu_rsq_lane_ops_per_s": peaks_live["mufu_rsq_lane_ops_per_s"],
         "measured_dfma_lane_ops_per_s": peaks_live["dfma_lane_ops_per_s"],
         "mufu_frac": pairs / (k_ms * 1e-3) / peaks_live["mufu_rsq_lane_ops_per_s"]}
-    if k == 4:          # the microbenchmarks behind DESIGN.md section 6 (register operands of packed instructions, trip-loop replica)
-        from paper_2110_11392_b200.opbench import operand_probe
-        out["roofline"]["operand_probe"] = operand_probe(sm_max)
     out["stage_ms"] = {kk: statistics.mean(st[kk] for st in stage_acc) for kk in stage_acc[0]}
     if args.neighbours:
         out["neighbour_steps"] = _neighbour_steps(nf, d_pos, d_acc, cfg, peaks_live)

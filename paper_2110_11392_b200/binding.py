@@ -161,6 +161,7 @@ class NearField:
             raise NearFieldError(rc, _L.nf_last_error(None).decode())
         self.cpd, self.R, self.eps_plummer, self.box = int(cpd), int(R), float(eps_plummer), float(box)
         self._N = 0
+        self._pinned = None          # the tensor nf_bin / nf_rebin pinned (kept alive: the pin is keyed on its address)
 
     # -- helpers
     def _check(self, rc: int):
@@ -213,13 +214,18 @@ class NearField:
         self._check(_L.nf_set_softening(self._h, {"spline": 0, "plummer": 1, "newton": 2}[law]))
 
     def bin(self, pos, stream=None):
-        """nf_bin: sort ``pos`` into grid order now and keep the binning for the following calls on ``pos``."""
+        """nf_bin: sort ``pos`` into grid order now and keep the binning for the following calls on ``pos``.
+        The library recognises the pinned buffer by its address and length alone.  This wrapper therefore keeps a
+        reference to ``pos`` while it is pinned, so that torch's caching allocator cannot hand the same address to a
+        new tensor of the same size (which would silently be served the old grid order).  Changing ``pos`` in place
+        by anything but ``kick_drift`` is still the caller's to announce: ``unbin()`` or ``bin()`` again."""
         import torch
         if not (pos.is_cuda and pos.dtype == torch.float32 and pos.is_contiguous() and pos.dim() == 2 and pos.shape[1] == 3):
             raise ValueError("pos must be a contiguous CUDA float32 tensor of shape [N,3]")
         st = torch.cuda.current_stream(pos.device) if stream is None else stream
         self._N = pos.shape[0]
         self._check(_L.nf_bin(self._h, pos.data_ptr(), pos.shape[0], ctypes.c_void_p(st.cuda_stream)))
+        self._pinned = pos
 
     def rebin(self, pos, stream=None):
         """nf_rebin: update the kept grid order after the particles moved (insert list + merge) and pin it."""
@@ -229,9 +235,11 @@ class NearField:
         st = torch.cuda.current_stream(pos.device) if stream is None else stream
         self._N = pos.shape[0]
         self._check(_L.nf_rebin(self._h, pos.data_ptr(), pos.shape[0], ctypes.c_void_p(st.cuda_stream)))
+        self._pinned = pos
 
     def unbin(self):
         self._check(_L.nf_unbin(self._h))
+        self._pinned = None
 
     def delivered_pairs(self):
         """nf_debug_delivered_pairs -> (deliveries incl. self meetings, self meetings) of the last accel."""

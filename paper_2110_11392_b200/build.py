@@ -133,17 +133,18 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_debug_library(out: str, verbose: bool = False) -> str:
-    """The -DNF_DEBUG_BOUNDS build of the product library (csrc/nf_common.cuh: every derived index is checked
-    against the bound of its array; nf_sync reports a violation), written to ``out`` -- never over the
-    in-tree library.  tests/test_gpu_debug_bounds.py runs the small parity cases under it."""
+def build_debug_library(out: str, verbose: bool = False, defines: tuple[str, ...] = ("-DNF_DEBUG_BOUNDS",)) -> str:
+    """A build of the product library with other ``defines``, written to ``out`` -- never over the in-tree library.
+    Default: the -DNF_DEBUG_BOUNDS build (csrc/nf_common.cuh: every derived index is checked against the bound of
+    its array; nf_sync reports a violation); tests/test_gpu_debug_bounds.py runs the small parity cases under it.
+    tests/test_gpu_ring_stress.py builds the copy-ring stress variants (-DNF_NSTAGE=2 -DNF_REFILL_BELOW=1, ...)."""
     nvcc = os.environ.get("NVCC", "nvcc")
     objdir = out + ".obj"
     os.makedirs(objdir, exist_ok=True)
 
     def one(src: str) -> str:
         obj = os.path.join(objdir, src.replace(os.sep, "_") + ".o")
-        cmd = [nvcc, *NVCC_FLAGS, "-DNF_DEBUG_BOUNDS", "-c", "-o", obj, os.path.join(CSRC, src)]
+        cmd = [nvcc, *NVCC_FLAGS, *defines, "-c", "-o", obj, os.path.join(CSRC, src)]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.run(cmd, check=True, stdout=sys.stderr, stderr=sys.stderr)

@@ -79,6 +79,8 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     TRY_ALLOC(c->d_pairs, 64);      // [0..1] pair counter, sink counter; [2..4] time-step reduction (doubles)
     TRY_ALLOC(c->d_nbr, (size_t)4 * 729 * 4);
 #undef TRY_ALLOC
+    // flags and counters start at zero (nf_cell_histogram only ever SETS the bad-position flag ctrl[2], and may be the first call)
+    if (cudaMemset(c->d_ctrl, 0, 128 * 4) != cudaSuccess) { snprintf(c->err, sizeof c->err, "nf_create: cudaMemset failed"); return fail(NF_ECUDA); }
     for (int i = 0; i < 8; ++i)
         if (cudaEventCreate(&c->ev[i]) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaEventCreate failed"); return fail(NF_ECUDA); }
     if (cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
@@ -87,6 +89,7 @@ extern "C" nf_status nf_create(nf_ctx **out, int cpd, int R, double eps_plummer,
     for (int i = 0; i < NF_HOST_CHUNKS; ++i)
         if (cudaEventCreateWithFlags(&c->ev_chunk[i], cudaEventDisableTiming) != cudaSuccess) { snprintf(c->err, sizeof c->err, "cudaEventCreate failed"); return fail(NF_ECUDA); }
     rc = nf_interact_setup(c);
+    if (rc == NF_OK) rc = nf_binner_setup(c);
     if (rc != NF_OK) return fail(rc);
     *out = c;
     return NF_OK;
@@ -175,7 +178,7 @@ static nf_status ensure_scratch(nf_ctx *c, int64_t N) {
     const int64_t capBlk = capPad / NF_BS + c->ncol + 8;
     cudaError_t e = cudaSuccess;
     auto A = [&](void **p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
-    A((void **)&c->d_key, (size_t)N * 4);
+    A((void **)&c->d_key, (size_t)(N < 8 ? 8 : N) * 4);      // (also nf_select_slabs' block counts + scan: 2 (ceil(N/256) + 1) words, more than N when N <= 3)
     A((void **)&c->d_arr, (size_t)N * 4);
     A((void **)&c->d_tmp_perm, (size_t)capPad * 4);
     A((void **)&c->d_chunk_sorted, (size_t)capPad * 4);
@@ -349,7 +352,7 @@ static nf_status accel_any(nf_ctx *c, const float *d_pos, int64_t N, float *d_ac
     if (c->opt_stage_timing) cudaEventRecord(c->ev[4], st);
     const double gm = c->gm > 0 ? c->gm : 1.0 / (double)N;
     const double cellsz = c->box / (double)c->cpd;
-    const float kfac = (float)(gm / (cellsz * cellsz));
+    const double kfac = gm / (cellsz * cellsz);
     rc = nf_run_interact(c, d_pos, N, d_acc, ostride, kfac, st);
     if (rc != NF_OK) return rc;
     c->have_sched = 1;

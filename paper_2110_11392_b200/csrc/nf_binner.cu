@@ -312,6 +312,12 @@ __global__ void __launch_bounds__(256) k_rank_big(const float *__restrict__ pos,
     }
 }
 
+// once per context (nf_create): k_sort_big's second launch needs 128 KB of dynamic shared memory
+nf_status nf_binner_setup(nf_ctx *ctx) {
+    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_sort_big, cudaFuncAttributeMaxDynamicSharedMemorySize, NF_SORT_MAX * 4));
+    return NF_OK;
+}
+
 // A2 + A3 once the histogram of all N particles is complete on `st`
 static nf_status binner_finish(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st) {
     const uint32_t n = (uint32_t)N;
@@ -330,7 +336,6 @@ static nf_status binner_finish(nf_ctx *ctx, const float *d_pos, int64_t N, cudaS
                                                                    ctx->d_perm_true, ctx->d_perm_pad, ctx->d_chunk_sorted, ctx->d_key); ctx->launches++;
     // (d_key is free after the scatter: it holds the worklist of long cells, at most N / NF_RANK_CHUNK entries)
     // two launches: the many cells of up to 8192 particles at 32 KB of shared memory (6 CTAs per SM), the few up to NF_SORT_MAX at 128 KB
-    NF_CUDA_OK(ctx, cudaFuncSetAttribute(k_sort_big, cudaFuncAttributeMaxDynamicSharedMemorySize, NF_SORT_MAX * 4));
     k_sort_big<<<ctx->sm_count * 6, 256, 8192 * 4, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,
                                                         ctx->d_tmp_perm, ctx->d_key, ctx->d_sorted, ctx->d_perm_true, ctx->d_perm_pad, NF_RANK_CHUNK, 8192u); ctx->launches++;
     k_sort_big<<<ctx->sm_count, 1024, NF_SORT_MAX * 4, st>>>(d_pos, ctx->prm.scale, (uint32_t)ctx->capPad, ctx->d_ctrl, ctx->d_offsets, ctx->d_poff,

@@ -143,7 +143,7 @@ nf_status nf_run_binner_host(nf_ctx *ctx, const float *h_pos, float *d_pos, int6
 nf_status nf_run_rebin(nf_ctx *ctx, const float *d_pos, int64_t N, cudaStream_t st);
 nf_status nf_scan_cells(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_run_scheduler(nf_ctx *ctx, int64_t N, cudaStream_t st);
-nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st);
+nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, double kfac, cudaStream_t st);
 nf_status nf_run_neighbors(nf_ctx *ctx, int cell, cudaStream_t st);
 nf_status nf_run_multipoles(nf_ctx *ctx, const float *d_pos, int order, double *d_M, cudaStream_t st);
 nf_status nf_run_kick_drift(nf_ctx *ctx, float *d_pos, float *d_vel, const float *d_acc, int64_t N, double dt_kick, double dt_drift,
@@ -157,6 +157,7 @@ nf_status nf_run_cell_histogram(nf_ctx *ctx, const float *d_pos, int64_t N, int3
 nf_status nf_run_slab_pairs(nf_ctx *ctx, const int32_t *d_counts, long long *d_pairs, long long *d_npart, cudaStream_t st);
 nf_status nf_run_select_slabs(nf_ctx *ctx, const float *d_pos, int64_t N, int x0, int nx, float *d_out, uint32_t *d_blk, cudaStream_t st);
 nf_status nf_interact_setup(nf_ctx *ctx);
+nf_status nf_binner_setup(nf_ctx *ctx);
 nf_status nf_scan_pairs(nf_ctx *ctx, cudaStream_t st);
 nf_status nf_scan_u32(nf_ctx *ctx, const uint32_t *in, uint32_t n, uint32_t *out, cudaStream_t st);
 

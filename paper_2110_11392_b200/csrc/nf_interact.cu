@@ -280,10 +280,11 @@ struct InteractArgs {
     uint32_t *ctrl;
     const float *dyn;        // [0] rc^2 (cell units^2; 0 = no close-pair radius, use the min form)  [1] rc  [2] rc^-3
     float *acc;
-    float kfac;
+    double kfac;             // gm / cell^2 (cell units -> length units); double: a float here is a relative error of up to 6e-8
+                             // on EVERY acceleration, i.e. 1.2e-5 rms on a sink pulled at 200 rms by a close neighbour
     float addend;            // addend of r^2: NF_TAU (spline) or eps_p^2 in cell units (Plummer, Eq. 2)
     float b2;                // density radius^2 (cell units) + addend; DENS only
-    float wfac;              // cell^2: density sum to length units
+    double wfac;             // cell^2: density sum to length units
     int ostride;             // floats per output particle: 3, or 4 with the density estimate in the 4th
     int near_cheb;           // cells within this Chebyshev distance run the near-cell form
     double close_eps;        // eps_s in cell units for close_scan's Eq. 3 branch (0: no softening, NF_SOFT_NEWTON)
@@ -856,11 +857,11 @@ __global__ void __launch_bounds__(NF_CTA_THREADS, NF_MIN_CTAS) k_interact(const 
                     NF_CHECK(A.ctrl, dst == 0xffffffffu || dst < A.n_part, 7);
                     if (dst != 0xffffffffu) {
                         float *o = A.acc + (size_t)A.ostride * dst;
-                        o[0] = (float)((double)A.kfac * ((double)tot[0][tid_s + j] + close_corr[0][tid_s + j]));
-                        o[1] = (float)((double)A.kfac * ((double)tot[1][tid_s + j] + close_corr[1][tid_s + j]));
-                        o[2] = (float)((double)A.kfac * ((double)tot[2][tid_s + j] + close_corr[2][tid_s + j]));
+                        o[0] = (float)(A.kfac * ((double)tot[0][tid_s + j] + close_corr[0][tid_s + j]));
+                        o[1] = (float)(A.kfac * ((double)tot[1][tid_s + j] + close_corr[1][tid_s + j]));
+                        o[2] = (float)(A.kfac * ((double)tot[2][tid_s + j] + close_corr[2][tid_s + j]));
                         // density: the sink met itself exactly once (r = 0 -> b^2); take that off (reading D1)
-                        if (DENS) o[3] = (float)((double)A.wfac * ((double)tot[DENS ? 6 : 0][tid_s + j] - ((double)A.b2 - (double)A.addend)));
+                        if (DENS) o[3] = (float)(A.wfac * ((double)tot[DENS ? 6 : 0][tid_s + j] - ((double)A.b2 - (double)A.addend)));
                     }
                 }
             }
@@ -911,7 +912,7 @@ nf_status nf_interact_setup(nf_ctx *ctx) {
     return NF_OK;
 }
 
-static void fill_interact_args(nf_ctx *ctx, const float *d_pos, float *d_out, int ostride, float kfac, InteractArgs &A, int &law, int &dens) {
+static void fill_interact_args(nf_ctx *ctx, const float *d_pos, float *d_out, int ostride, double kfac, InteractArgs &A, int &law, int &dens) {
     (void)d_pos;
     A.sx = ctx->d_sorted; A.sy = ctx->d_sorted + ctx->capPad; A.sz = ctx->d_sorted + 2ull * ctx->capPad;
     A.lx = ctx->d_sorted + 4ull * ctx->capPad; A.ly = ctx->d_sorted + 5ull * ctx->capPad; A.lz = ctx->d_sorted + 6ull * ctx->capPad;
@@ -932,7 +933,7 @@ static void fill_interact_args(nf_ctx *ctx, const float *d_pos, float *d_out, in
     const double bc = ctx->dens_b * ctx->prm.scale;           // density radius in cell units
     A.b2 = (float)(bc * bc) + A.addend;
     const double cellsz = ctx->box / (double)ctx->cpd;
-    A.wfac = (float)(cellsz * cellsz);
+    A.wfac = cellsz * cellsz;
     // near cells: may hold r < eps_s (spline), r < r_c <= 0.25 (Plummer, Newton), or r < b (density)
     int nc = ctx->law == NF_SOFT_SPLINE ? ctx->prm.near_cheb : 1;
     if (dens) { const int nb = (int)ceil(bc); if (nb > nc) nc = nb; }
@@ -941,7 +942,7 @@ static void fill_interact_args(nf_ctx *ctx, const float *d_pos, float *d_out, in
 }
 
 // d_out: N x ostride floats (ostride 3: accelerations; 4: accelerations + density estimate)
-nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, float kfac, cudaStream_t st) {
+nf_status nf_run_interact(nf_ctx *ctx, const float *d_pos, int64_t N, float *d_out, int ostride, double kfac, cudaStream_t st) {
     InteractArgs A;
     int law, dens;
     fill_interact_args(ctx, d_pos, d_out, ostride, kfac, A, law, dens);

@@ -153,13 +153,17 @@ __device__ __forceinline__ void mp_all_slices(const MultipoleArgs &A, uint32_t p
 // its exclusive scan (k_mp_scan), then the running cursors of k_mp_fill; hist[NFM_NCLASS] = number of items;
 // hist[NFM_CTR_CHUNK] / hist[NFM_CTR_DENSE] count the chunks and the dense cells.  The order within a class
 // is whatever the atomics give: which lane computes an item does not change its result.
-// A dense cell (n > NFM_LANE_MAX = 2 NFM_CHUNK) has ceil(n / NFM_CHUNK) <= 3 n / (2 NFM_LANE_MAX) chunks, so
-// all chunks of any input fit the partial buffer (the binner's chunk scratch: 4 capPad bytes >= N / 330 chunks).
+// A dense cell (n > NFM_LANE_MAX = 2 NFM_CHUNK) has ceil(n / NFM_CHUNK) chunks; chunks per particle are most at
+// n = NFM_LANE_MAX + 1 (3 chunks for 1025 particles), so the partials of any input take at most
+// 3 * 165 * 8 B / 1025 = 3.87 B per particle of a dense cell -- inside the partial buffer (the binner's chunk
+// scratch: 4 capPad bytes >= 4 B per particle) with 3 % to spare; the static_assert below keeps it so.
 #define NFM_CHUNK 512
 #define NFM_NCLASS (NFM_LANE_MAX + 1)
 #define NFM_CTR_CHUNK (NFM_NCLASS + 1)
 #define NFM_CTR_DENSE (NFM_NCLASS + 2)
 static_assert(NFM_LANE_MAX == 2 * NFM_CHUNK, "the bound on the number of chunks assumes it");
+static_assert(((NFM_LANE_MAX + 1 + NFM_CHUNK - 1) / NFM_CHUNK) * 165 * 8 <= 4 * (NFM_LANE_MAX + 1),
+              "the order-8 chunk partials (165 doubles per chunk) must fit 4 bytes per particle of a dense cell");
 __device__ __forceinline__ uint32_t mp_class(uint32_t cnt) { return NFM_LANE_MAX - cnt; }   // longest first
 __global__ void __launch_bounds__(256) k_mp_hist(int ncell, const uint32_t *__restrict__ offsets, uint32_t *__restrict__ hist) {
     __shared__ uint32_t h[NFM_NCLASS];

@@ -86,7 +86,8 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_write(const float *__res
 
 nf_status nf_run_cell_histogram(nf_ctx *ctx, const float *d_pos, int64_t N, int32_t *d_counts, cudaStream_t st) {
     NF_CUDA_OK(ctx, cudaMemsetAsync(d_counts, 0, (size_t)ctx->ncell * sizeof(int32_t), st));
-    NF_CUDA_OK(ctx, cudaMemsetAsync(ctx->d_ctrl + 2, 0, sizeof(uint32_t), st));
+    // (the bad-position flag ctrl[2] is only ever SET here: a flag still pending from an earlier call that nf_sync has
+    //  not reported yet must survive; the binner's reset at the start of each sort and nf_create's zero-fill clear it)
     if (N > 0) { k_cell_hist<<<(uint32_t)((N + 255) / 256), 256, 0, st>>>(d_pos, (uint32_t)N, ctx->prm.scale, ctx->cpd, d_counts, ctx->d_ctrl); ctx->launches++; }
     NF_CUDA_OK(ctx, cudaGetLastError());
     return NF_OK;

@@ -211,7 +211,16 @@ class SlabNearField:
         self.n_ghost = int(ghosts.shape[0])
         self.halo_bytes = self.n_ghost * 12
         n_tot = n_own + self.n_ghost
+        # The copy into _buf, the slab selection and the halo receive ran on torch's CURRENT stream; the force call
+        # runs on ``stream``.  When the two differ they are ordered here in both directions: the force waits for
+        # own + ghost rows to be complete, and the current stream waits for the force, so that the returned view (and
+        # the next call's writes into _buf / _acc) are safe for a caller that keeps working on the current stream.
+        cur = torch.cuda.current_stream(pos_own.device) if pos_own.is_cuda else None
+        if stream is not None and cur is not None and stream != cur:
+            stream.wait_stream(cur)
         self.nf.accel(self._buf[:n_tot], self._acc[:n_tot], stream=stream)      # ghost rows of acc are not written
+        if stream is not None and cur is not None and stream != cur:
+            cur.wait_stream(stream)
         return self._acc[:n_own]
 
     def interaction_count(self) -> int:

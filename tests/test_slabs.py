@@ -176,6 +176,38 @@ def test_cell_histogram_slab_pairs_and_select_match_the_oracle(oracle_mod):
         assert bounds == slabs.balance_slabs(pairs, 3) and sum(nx for _, nx in bounds) == cfg.cpd
 
 
+@pytest.mark.gpu
+def test_histogram_keeps_a_pending_bad_position_flag_and_tiny_selections_work():
+    """ nf_cell_histogram used to clear the NaN/Inf flag of an earlier call that nf_sync had not reported
+    yet; and nf_select_slabs' block scratch was larger than the N words it borrowed when N <= 3."""
+    from paper_2110_11392_b200.binding import NearField, NearFieldError, NF_EPOS
+    good = torch.from_numpy(W.uniform(2000, 3)).cuda()
+    bad = good.clone()
+    bad[17, 1] = float("inf")
+    with NearField(7, 2, 1e-3, 1.0) as nf:
+        c0 = nf.cell_histogram(good)               # first call on a fresh context: flag starts at zero
+        nf.sync()
+        assert int(c0.sum()) == 2000
+        nf.bin(bad)                                # sets the flag ...
+        c1 = nf.cell_histogram(good)               # ... which this call must not clear
+        assert int(c1.sum()) == 2000
+        with pytest.raises(NearFieldError) as e:
+            nf.sync()
+        assert e.value.status == NF_EPOS
+        c2 = nf.cell_histogram(bad)                # the histogram's own detection: not counted, reported
+        with pytest.raises(NearFieldError):
+            nf.sync()
+        assert int(c2.sum()) == 1999
+        nf.bin(good)                               # a new sort starts clean
+        nf.sync()
+    for n in (1, 2, 3, 4):
+        with NearField(7, 2, 1e-3, 1.0) as nf:     # fresh context: scratch sized for exactly n particles
+            p = good[:n].contiguous()
+            out = torch.empty_like(p)
+            assert nf.select_slabs(p, 0, 7, out=out) == n and torch.equal(out, p)
+            assert nf.select_slabs(p, 0, 0) == 0
+
+
 # ----------------------------------------------------------------------------- GPU: emulated decomposition
 @pytest.mark.gpu
 @pytest.mark.parametrize("label,cfg,world", [("cfg2@13 x3", W.scaled(W.CONFIGS[2], 13), 3),
@@ -248,6 +280,28 @@ def test_slab_nearfield_single_rank_equals_plain_call():
     with pytest.raises(ValueError):
         half.accel(pos, validate=True)
     half.close()
+
+
+@pytest.mark.gpu
+def test_slab_nearfield_on_a_side_stream_is_ordered_with_the_current_stream():
+    """accel(stream=side): the internal copy of pos_own runs on the current stream and the force on ``side``.
+    The call orders the two itself (it did not), so a caller that keeps working on the current
+    stream -- changing pos_own right after the call, reading the result without a sync of ``side`` -- is safe."""
+    from paper_2110_11392_b200.binding import NearField
+    cfg = W.scaled(W.CONFIGS[2], 21)              # 370 k particles: the copy and the force take long enough to overlap
+    pos = torch.from_numpy(W.make_positions(cfg)).cuda()
+    with NearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0) as nf:
+        ref = nf.accel(pos).clone()
+        nf.sync()
+    side = torch.cuda.Stream()
+    snf = slabs.SlabNearField(cfg.cpd, cfg.R, cfg.eps_p, 1.0, [(0, cfg.cpd)], gm=1.0 / cfg.N)
+    for _ in range(3):
+        work = pos.clone()
+        a = snf.accel(work, stream=side)
+        got = a.clone()                           # current stream, no explicit sync with ``side``
+        work.zero_()                              # the caller's buffer is its own again
+        assert torch.equal(got, ref)
+    snf.close()
 
 
 @pytest.mark.gpu
